@@ -1,0 +1,134 @@
+/*
+ * das.h -- C ABI of the B200-native volumetric delay-and-sum (DAS) beamformer.
+ *
+ * The library computes, for every voxel p_n of a rectilinear grid,
+ *
+ *     x_n = sum_q sum_m  w_rx(m,n) * y_qm[ t_qmn ] * R(tau_qmn)                       (Eq. 2)
+ *
+ *     tau_qmn = tau_tx(q,n) + |p_n - r_m| / c                    (Eq. 1)
+ *     tau_tx  = (p_n . u_q)/c + t0_q          plane wave          (fn. 2; sign
+ *             = |p_n - v_q|/c + t0_q          diverging wave       and t0 per DESIGN.md A1/A2)
+ *     t_qmn   = (tau_qmn - t_start) * fs,  y[t] = (1-a) y[k] + a y[k+1], k = floor(t), a = t-k
+ *               (linear interpolation); the term is dropped unless 0 <= k <= K-2
+ *     w_rx    = 1 if f_number <= 0, else 1 iff a > 0 and 4 f#^2 rho^2 <= a^2 with
+ *               a = (p_n - r_m).n_m, rho^2 = |p_n - r_m|^2 - a^2   (f-number boxcar on a cone
+ *               about the element normal; "origin and a direction")
+ *     R(tau)  = exp(+j 2 pi fc tau) for IQ data (BASELINE.json north_star), 1 for RF data
+ *
+ * All delays are computed in-kernel; nothing of size N*M*Q is ever stored.
+ * Accumulation is FP32 whatever the storage precision.
+ *
+ * Conventions
+ *   - Plain C, no exceptions cross this boundary; every call returns a das_status_t
+ *     (or a size / string).  das_last_error() gives a thread-local detail string.
+ *   - "host" / "device" on a pointer says where the memory lives.  Device pointers must
+ *     belong to the plan's CUDA device.  The library never takes ownership of caller memory.
+ *   - das_convert / das_execute only enqueue work on the given CUDA stream (a cudaStream_t
+ *     passed as void*; NULL = the legacy default stream).  They never synchronise and never
+ *     allocate.  A plan is immutable after creation: concurrent das_execute calls on
+ *     different streams with different buffers are allowed.
+ */
+#ifndef DAS_B200_H_
+#define DAS_B200_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct das_plan das_plan_t;      /* opaque, owned by the library */
+
+typedef enum {
+  DAS_OK = 0,
+  DAS_ERR_INVALID_ARG = 1,   /* null pointer, size < 1, non-finite or non-positive c / fs, ... */
+  DAS_ERR_UNSUPPORTED = 2,   /* unknown enum value or a combination this build does not implement */
+  DAS_ERR_ALLOC = 3,         /* host or device allocation failed */
+  DAS_ERR_CUDA = 4,          /* a CUDA runtime call or kernel launch failed (see das_last_error) */
+  DAS_ERR_SIZE = 5           /* problem exceeds an internal limit (index overflow) */
+} das_status_t;
+
+typedef enum { DAS_TX_PLANE = 0, DAS_TX_DIVERGING = 1 } das_tx_type_t;
+typedef enum { DAS_DATA_IQ = 0, DAS_DATA_RF = 1 } das_data_kind_t;
+typedef enum { DAS_STORE_FP32 = 0, DAS_STORE_FP16 = 1 } das_storage_t;
+typedef enum {
+  DAS_ALGO_AUTO = 0,     /* tiled kernel when the geometry allows it, else the general kernel */
+  DAS_ALGO_GENERAL = 1,  /* one thread per voxel, any element positions / normals (Alg. 1 shape) */
+  DAS_ALGO_TILED = 2     /* voxel-tiled, shared-memory staged kernel; needs a planar array with
+                            all normals (0,0,1); DAS_ERR_UNSUPPORTED otherwise */
+} das_algo_t;
+
+/* One transmit event (one "observation" q of the paper). */
+typedef struct {
+  int   type;      /* das_tx_type_t */
+  float v[3];      /* PLANE: unit propagation direction u_q.  DIVERGING: virtual source v_q [m] */
+  float t0;        /* seconds added to tau_tx (time-zero convention, reading A2) */
+} das_transmit_t;
+
+/* Everything that defines a reconstruction except the channel data.  All pointers are HOST
+ * pointers; the plan copies what it needs, the caller may free them after das_plan_create. */
+typedef struct {
+  const float* elem_pos;  int n_elem;   /* [M][3] receiver positions r_m, metres */
+  const float* elem_dir;                /* [M][3] unit normals n_m, or NULL = (0,0,1) for all */
+  const das_transmit_t* tx; int n_tx;   /* [Q] */
+  const float* xs; int nx;              /* axis vectors of the rectilinear voxel grid, metres; */
+  const float* ys; int ny;              /*   voxel (ix,iy,iz) sits at (xs[ix], ys[iy], zs[iz])  */
+  const float* zs; int nz;
+  float c;            /* speed of sound c0 [m/s], > 0 */
+  float fc;           /* demodulation frequency [Hz] for the IQ phase rotation, >= 0; must be 0 for RF */
+  float fs;           /* sampling rate of the channel data [Hz], > 0 */
+  float t_start;      /* time of sample k = 0 [s] */
+  float f_number;     /* receive f-number of the boxcar apodization; <= 0 disables apodization */
+  int   n_samples;    /* K >= 2, samples per (transmit, element) */
+  int   data_kind;    /* das_data_kind_t: IQ = complex64 in, complex64 out; RF = float32 in/out */
+  int   storage;      /* das_storage_t: precision of the converted (device-layout) channel data */
+  int   algo;         /* das_algo_t */
+  int   device;       /* CUDA device ordinal */
+  int   n_frames;     /* reserved for a frame batch; must be 0 or 1 */
+} das_plan_desc_t;
+
+/* Validates *desc, uploads geometry and small derived tables to desc->device, chooses launch
+ * shapes.  On success *out_plan is a new plan (free with das_plan_destroy). */
+das_status_t das_plan_create(const das_plan_desc_t* desc, das_plan_t** out_plan);
+das_status_t das_plan_destroy(das_plan_t* plan);            /* NULL is allowed */
+
+size_t das_raw_bytes(const das_plan_t* plan);        /* Q*M*K * (8 for IQ, 4 for RF)              */
+size_t das_converted_bytes(const das_plan_t* plan);  /* size of the buffer das_convert writes      */
+size_t das_output_bytes(const das_plan_t* plan);     /* nx*ny*nz * (8 for IQ, 4 for RF)            */
+int    das_plan_algo(const das_plan_t* plan);        /* the das_algo_t actually selected           */
+
+/* Layout transform + cast (the paper's permute-and-convert pre-pass).
+ *   d_raw   device, [Q][M][K] complex64 (re,im interleaved) for IQ or float32 for RF,
+ *           samples contiguous in k (the paper's layout with B = 1)
+ *   d_conv  device, das_converted_bytes() bytes, 16-byte aligned; written entirely
+ *   scale   every sample is multiplied by it before the cast (1.0f = none); lets the caller
+ *           keep fp16 storage inside its normal range
+ * fp16 storage rounds to nearest even; overflow gives +-inf (reading A11). */
+das_status_t das_convert(const das_plan_t* plan, const void* d_raw, void* d_conv, float scale,
+                         void* stream);
+
+/* Beamform one volume.
+ *   d_conv  device, produced by das_convert with this plan (or a plan with identical
+ *           n_tx, n_elem, n_samples, data_kind and storage)
+ *   d_out   device, das_output_bytes() bytes, [nx][ny][nz] with z fastest (C order), complex64
+ *           (IQ) or float32 (RF); overwritten, not accumulated into; 8-byte aligned */
+das_status_t das_execute(const das_plan_t* plan, const void* d_conv, void* d_out, void* stream);
+
+/* End-to-end convenience for HOST buffers: copies h_raw to the device, runs das_convert
+ * (scale 1) and das_execute, copies the volume back to h_out and synchronises the stream
+ * before returning.  Uses device staging buffers owned by the plan (allocated on first use and
+ * freed by das_plan_destroy), therefore NOT safe to call concurrently on one plan.  For full
+ * copy bandwidth h_raw / h_out should be page-locked. */
+das_status_t das_beamform_host(das_plan_t* plan, const void* h_raw, void* h_out, void* stream);
+
+const char* das_status_string(das_status_t s);
+const char* das_last_error(void);        /* thread-local, never NULL */
+
+/* Number of kernels the library has launched in this process (all plans, all threads).
+ * The bench reports it as gpu_launches. */
+unsigned long long das_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DAS_B200_H_ */

@@ -1,0 +1,295 @@
+// C ABI of libdas_b200.so (include/das.h): plan creation / validation, dispatch, errors.
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "das_internal.cuh"
+
+namespace das {
+
+static std::atomic<unsigned long long> g_launches{0};
+void count_launch(unsigned long long n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+static thread_local char g_err[512] = "";
+
+static void set_err(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+static das_status_t cuda_fail(cudaError_t e, const char* what) {
+  set_err("%s: %s (%s)", what, cudaGetErrorString(e), cudaGetErrorName(e));
+  return DAS_ERR_CUDA;
+}
+
+// Restores the caller's current device on scope exit.
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = false;
+  cudaError_t err = cudaSuccess;
+  explicit DeviceGuard(int dev) {
+    err = cudaGetDevice(&prev);
+    if (err != cudaSuccess) return;
+    if (prev != dev) {
+      err = cudaSetDevice(dev);
+      if (err != cudaSuccess) return;
+    }
+    ok = true;
+  }
+  ~DeviceGuard() { if (ok && prev >= 0) cudaSetDevice(prev); }
+};
+
+}  // namespace das
+
+using namespace das;
+
+struct das_plan {
+  Params P{};
+  int device = 0;
+  int algo = DAS_ALGO_GENERAL;
+  size_t raw_bytes = 0, conv_bytes = 0, out_bytes = 0;
+  std::vector<void*> dev_allocs;          // geometry tables
+  TiledPlan* tiled = nullptr;
+  // staging for das_beamform_host (lazy)
+  void* st_raw = nullptr;
+  void* st_conv = nullptr;
+  void* st_out = nullptr;
+};
+
+static void free_plan(das_plan* p) {
+  if (!p) return;
+  DeviceGuard g(p->device);
+  if (p->tiled) tiled_plan_destroy(p->tiled);
+  for (void* d : p->dev_allocs) cudaFree(d);
+  if (p->st_raw) cudaFree(p->st_raw);
+  if (p->st_conv) cudaFree(p->st_conv);
+  if (p->st_out) cudaFree(p->st_out);
+  delete p;
+}
+
+template <typename T>
+static cudaError_t upload(das_plan* p, const std::vector<T>& h, const T** d_out) {
+  void* d = nullptr;
+  cudaError_t e = cudaMalloc(&d, h.size() * sizeof(T));
+  if (e != cudaSuccess) return e;
+  p->dev_allocs.push_back(d);
+  e = cudaMemcpy(d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice);
+  *d_out = static_cast<const T*>(d);
+  return e;
+}
+
+static bool finite_all(const float* p, long long n) {
+  for (long long i = 0; i < n; ++i) if (!std::isfinite(p[i])) return false;
+  return true;
+}
+
+extern "C" {
+#pragma GCC visibility push(default)
+
+const char* das_status_string(das_status_t s) {
+  switch (s) {
+    case DAS_OK: return "DAS_OK";
+    case DAS_ERR_INVALID_ARG: return "DAS_ERR_INVALID_ARG";
+    case DAS_ERR_UNSUPPORTED: return "DAS_ERR_UNSUPPORTED";
+    case DAS_ERR_ALLOC: return "DAS_ERR_ALLOC";
+    case DAS_ERR_CUDA: return "DAS_ERR_CUDA";
+    case DAS_ERR_SIZE: return "DAS_ERR_SIZE";
+  }
+  return "DAS_ERR_UNKNOWN";
+}
+
+const char* das_last_error(void) { return g_err; }
+
+unsigned long long das_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+das_status_t das_plan_create(const das_plan_desc_t* d, das_plan_t** out_plan) {
+  g_err[0] = 0;
+  if (!out_plan) { set_err("out_plan is NULL"); return DAS_ERR_INVALID_ARG; }
+  *out_plan = nullptr;
+  if (!d) { set_err("desc is NULL"); return DAS_ERR_INVALID_ARG; }
+  if (!d->elem_pos || !d->tx || !d->xs || !d->ys || !d->zs) {
+    set_err("elem_pos, tx, xs, ys, zs must be non-NULL"); return DAS_ERR_INVALID_ARG;
+  }
+  if (d->n_elem < 1 || d->n_tx < 1 || d->nx < 1 || d->ny < 1 || d->nz < 1) {
+    set_err("n_elem, n_tx, nx, ny, nz must be >= 1"); return DAS_ERR_INVALID_ARG;
+  }
+  if (d->n_samples < 2) { set_err("n_samples must be >= 2 (linear interpolation needs k and k+1)"); return DAS_ERR_INVALID_ARG; }
+  if (!(std::isfinite(d->c) && d->c > 0.f)) { set_err("c must be finite and > 0"); return DAS_ERR_INVALID_ARG; }
+  if (!(std::isfinite(d->fs) && d->fs > 0.f)) { set_err("fs must be finite and > 0"); return DAS_ERR_INVALID_ARG; }
+  if (!(std::isfinite(d->fc) && d->fc >= 0.f)) { set_err("fc must be finite and >= 0"); return DAS_ERR_INVALID_ARG; }
+  if (!std::isfinite(d->t_start)) { set_err("t_start must be finite"); return DAS_ERR_INVALID_ARG; }
+  if (!std::isfinite(d->f_number)) { set_err("f_number must be finite"); return DAS_ERR_INVALID_ARG; }
+  if (d->data_kind != DAS_DATA_IQ && d->data_kind != DAS_DATA_RF) { set_err("unknown data_kind %d", d->data_kind); return DAS_ERR_UNSUPPORTED; }
+  if (d->storage != DAS_STORE_FP32 && d->storage != DAS_STORE_FP16) { set_err("unknown storage %d", d->storage); return DAS_ERR_UNSUPPORTED; }
+  if (d->algo != DAS_ALGO_AUTO && d->algo != DAS_ALGO_GENERAL && d->algo != DAS_ALGO_TILED) { set_err("unknown algo %d", d->algo); return DAS_ERR_UNSUPPORTED; }
+  if (d->n_frames != 0 && d->n_frames != 1) { set_err("n_frames = %d: frame batches are not implemented (one frame per call)", d->n_frames); return DAS_ERR_UNSUPPORTED; }
+  if (d->data_kind == DAS_DATA_RF && d->fc != 0.f) { set_err("fc must be 0 for RF data (no phase rotation)"); return DAS_ERR_INVALID_ARG; }
+  if (!finite_all(d->elem_pos, 3LL * d->n_elem) || !finite_all(d->xs, d->nx) ||
+      !finite_all(d->ys, d->ny) || !finite_all(d->zs, d->nz) ||
+      (d->elem_dir && !finite_all(d->elem_dir, 3LL * d->n_elem))) {
+    set_err("non-finite geometry value"); return DAS_ERR_INVALID_ARG;
+  }
+  for (int q = 0; q < d->n_tx; ++q) {
+    const das_transmit_t& t = d->tx[q];
+    if (t.type != DAS_TX_PLANE && t.type != DAS_TX_DIVERGING) { set_err("tx[%d]: unknown type %d", q, t.type); return DAS_ERR_UNSUPPORTED; }
+    if (!finite_all(t.v, 3) || !std::isfinite(t.t0)) { set_err("tx[%d]: non-finite value", q); return DAS_ERR_INVALID_ARG; }
+    if (t.type == DAS_TX_PLANE) {
+      const double n2 = (double)t.v[0] * t.v[0] + (double)t.v[1] * t.v[1] + (double)t.v[2] * t.v[2];
+      if (std::fabs(std::sqrt(n2) - 1.0) > 1e-4) { set_err("tx[%d]: plane-wave direction is not a unit vector", q); return DAS_ERR_INVALID_ARG; }
+    }
+  }
+  if (d->elem_dir) {
+    for (int m = 0; m < d->n_elem; ++m) {
+      const float* v = d->elem_dir + 3 * m;
+      const double n2 = (double)v[0] * v[0] + (double)v[1] * v[1] + (double)v[2] * v[2];
+      if (std::fabs(std::sqrt(n2) - 1.0) > 1e-4) { set_err("elem_dir[%d] is not a unit vector", m); return DAS_ERR_INVALID_ARG; }
+    }
+  }
+  const long long N = (long long)d->nx * d->ny * d->nz;
+  const int Kp = padded_samples(d->n_samples);
+  const long long rows = (long long)d->n_elem * d->n_tx;
+  if (N > (1LL << 40) || rows * Kp > (1LL << 40)) { set_err("problem too large"); return DAS_ERR_SIZE; }
+
+  das_plan* p = new (std::nothrow) das_plan();
+  if (!p) { set_err("out of host memory"); return DAS_ERR_ALLOC; }
+  p->device = d->device;
+  Params& P = p->P;
+  P.M = d->n_elem; P.Q = d->n_tx; P.K = d->n_samples; P.Kp = Kp;
+  P.nx = d->nx; P.ny = d->ny; P.nz = d->nz;
+  P.iq = d->data_kind == DAS_DATA_IQ;
+  P.fp16 = d->storage == DAS_STORE_FP16;
+  P.apod = d->f_number > 0.f;
+  P.has_dir = d->elem_dir != nullptr;
+  P.c = d->c; P.fc = d->fc; P.fs = d->fs; P.t_start = d->t_start; P.fnum = d->f_number;
+  const size_t in_elem = P.iq ? 8 : 4;
+  const size_t st_elem = (P.iq ? 2 : 1) * 2 * (P.fp16 ? 2 : 4);   // (mid, slope) entry
+  p->raw_bytes = (size_t)rows * P.K * in_elem;
+  p->conv_bytes = (size_t)rows * Kp * st_elem;
+  p->out_bytes = (size_t)N * in_elem;
+
+  DeviceGuard g(d->device);
+  if (!g.ok) { das_status_t s = cuda_fail(g.err, "selecting the CUDA device"); delete p; return s; }
+
+  std::vector<float> hx(d->xs, d->xs + d->nx), hy(d->ys, d->ys + d->ny), hz(d->zs, d->zs + d->nz);
+  std::vector<float4> he(d->n_elem), hd;
+  for (int m = 0; m < d->n_elem; ++m) he[m] = make_float4(d->elem_pos[3 * m], d->elem_pos[3 * m + 1], d->elem_pos[3 * m + 2], 0.f);
+  if (d->elem_dir) {
+    hd.resize(d->n_elem);
+    for (int m = 0; m < d->n_elem; ++m) hd[m] = make_float4(d->elem_dir[3 * m], d->elem_dir[3 * m + 1], d->elem_dir[3 * m + 2], 0.f);
+  }
+  std::vector<TxDev> ht(d->n_tx);
+  for (int q = 0; q < d->n_tx; ++q) {
+    ht[q].type = d->tx[q].type; ht[q].pad = 0;
+    ht[q].vx = d->tx[q].v[0]; ht[q].vy = d->tx[q].v[1]; ht[q].vz = d->tx[q].v[2];
+    ht[q].t0 = d->tx[q].t0;
+  }
+  cudaError_t e;
+  if ((e = upload(p, hx, &P.xs)) != cudaSuccess || (e = upload(p, hy, &P.ys)) != cudaSuccess ||
+      (e = upload(p, hz, &P.zs)) != cudaSuccess || (e = upload(p, he, &P.elem)) != cudaSuccess ||
+      (e = upload(p, ht, &P.tx)) != cudaSuccess ||
+      (d->elem_dir && (e = upload(p, hd, &P.edir)) != cudaSuccess)) {
+    das_status_t s = (e == cudaErrorMemoryAllocation) ? DAS_ERR_ALLOC : DAS_ERR_CUDA;
+    cuda_fail(e, "uploading plan tables");
+    free_plan(p);
+    return s;
+  }
+
+  p->algo = DAS_ALGO_GENERAL;
+  if (d->algo != DAS_ALGO_GENERAL) {
+    char why[256] = "";
+    cudaError_t ce = cudaSuccess;
+    p->tiled = tiled_plan_create(P, *d, d->device, why, sizeof(why), &ce);
+    if (p->tiled) {
+      p->algo = DAS_ALGO_TILED;
+    } else if (ce != cudaSuccess) {
+      das_status_t s = cuda_fail(ce, "building the tiled plan");
+      free_plan(p);
+      return s;
+    } else if (d->algo == DAS_ALGO_TILED) {
+      set_err("tiled kernel not applicable: %s", why);
+      free_plan(p);
+      return DAS_ERR_UNSUPPORTED;
+    }
+  }
+  *out_plan = p;
+  return DAS_OK;
+}
+
+das_status_t das_plan_destroy(das_plan_t* plan) {
+  free_plan(plan);
+  return DAS_OK;
+}
+
+size_t das_raw_bytes(const das_plan_t* p) { return p ? p->raw_bytes : 0; }
+size_t das_converted_bytes(const das_plan_t* p) { return p ? p->conv_bytes : 0; }
+size_t das_output_bytes(const das_plan_t* p) { return p ? p->out_bytes : 0; }
+int das_plan_algo(const das_plan_t* p) { return p ? p->algo : -1; }
+
+das_status_t das_convert(const das_plan_t* p, const void* d_raw, void* d_conv, float scale, void* stream) {
+  if (!p || !d_raw || !d_conv) { set_err("das_convert: NULL argument"); return DAS_ERR_INVALID_ARG; }
+  if (!std::isfinite(scale)) { set_err("das_convert: scale must be finite"); return DAS_ERR_INVALID_ARG; }
+  if (reinterpret_cast<uintptr_t>(d_conv) % 16 || reinterpret_cast<uintptr_t>(d_raw) % 8) {
+    set_err("das_convert: d_conv must be 16-byte and d_raw 8-byte aligned"); return DAS_ERR_INVALID_ARG;
+  }
+  DeviceGuard g(p->device);
+  if (!g.ok) return cuda_fail(g.err, "selecting the CUDA device");
+  cudaError_t e = launch_convert(p->P, d_raw, d_conv, scale, static_cast<cudaStream_t>(stream));
+  if (e != cudaSuccess) return cuda_fail(e, "das_convert launch");
+  return DAS_OK;
+}
+
+das_status_t das_execute(const das_plan_t* p, const void* d_conv, void* d_out, void* stream) {
+  if (!p || !d_conv || !d_out) { set_err("das_execute: NULL argument"); return DAS_ERR_INVALID_ARG; }
+  if (reinterpret_cast<uintptr_t>(d_conv) % 16 || reinterpret_cast<uintptr_t>(d_out) % 8) {
+    set_err("das_execute: d_conv must be 16-byte and d_out 8-byte aligned"); return DAS_ERR_INVALID_ARG;
+  }
+  DeviceGuard g(p->device);
+  if (!g.ok) return cuda_fail(g.err, "selecting the CUDA device");
+  cudaError_t e;
+  if (p->algo == DAS_ALGO_TILED) {
+    int nl = 0;
+    e = launch_tiled(p->tiled, p->P, d_conv, d_out, static_cast<cudaStream_t>(stream), &nl);
+  } else {
+    e = launch_general(p->P, d_conv, d_out, static_cast<cudaStream_t>(stream));
+  }
+  if (e != cudaSuccess) return cuda_fail(e, "das_execute launch");
+  return DAS_OK;
+}
+
+das_status_t das_beamform_host(das_plan_t* p, const void* h_raw, void* h_out, void* stream) {
+  if (!p || !h_raw || !h_out) { set_err("das_beamform_host: NULL argument"); return DAS_ERR_INVALID_ARG; }
+  DeviceGuard g(p->device);
+  if (!g.ok) return cuda_fail(g.err, "selecting the CUDA device");
+  cudaError_t e;
+  if (!p->st_raw) {
+    if ((e = cudaMalloc(&p->st_raw, p->raw_bytes)) != cudaSuccess ||
+        (e = cudaMalloc(&p->st_conv, p->conv_bytes)) != cudaSuccess ||
+        (e = cudaMalloc(&p->st_out, p->out_bytes)) != cudaSuccess) {
+      cuda_fail(e, "allocating staging buffers");
+      if (p->st_raw) { cudaFree(p->st_raw); p->st_raw = nullptr; }
+      if (p->st_conv) { cudaFree(p->st_conv); p->st_conv = nullptr; }
+      if (p->st_out) { cudaFree(p->st_out); p->st_out = nullptr; }
+      return DAS_ERR_ALLOC;
+    }
+  }
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if ((e = cudaMemcpyAsync(p->st_raw, h_raw, p->raw_bytes, cudaMemcpyHostToDevice, s)) != cudaSuccess)
+    return cuda_fail(e, "host-to-device copy");
+  das_status_t st = das_convert(p, p->st_raw, p->st_conv, 1.0f, stream);
+  if (st != DAS_OK) return st;
+  st = das_execute(p, p->st_conv, p->st_out, stream);
+  if (st != DAS_OK) return st;
+  if ((e = cudaMemcpyAsync(h_out, p->st_out, p->out_bytes, cudaMemcpyDeviceToHost, s)) != cudaSuccess)
+    return cuda_fail(e, "device-to-host copy");
+  if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return cuda_fail(e, "stream synchronize");
+  return DAS_OK;
+}
+
+#pragma GCC visibility pop
+}  // extern "C"

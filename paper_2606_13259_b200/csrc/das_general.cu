@@ -1,0 +1,149 @@
+// General delay-and-sum kernel: one thread per voxel, any receiver positions and normals.
+//
+// This is the computation of the paper's Algorithm 1 with B = 1, except that
+// the transmit delay is also computed in-kernel (BASELINE.json north_star) and the loops are
+// swapped (receiver outer, transmit inner, in chunks of kQc transmits) so that the receive
+// geometry is evaluated once per (m, n) instead of once per (q, m, n).  It is the fallback for
+// geometries the tiled kernel does not take (non-planar arrays, tilted normals) and the
+// reference point the tiled kernel is measured against; it is not the fast path.
+//
+// The channel data is read from the (mid, slope) table layout das_convert writes
+// (das_internal.cuh): one aligned load per term.
+//
+// Precision: all geometry (delays, aperture test, sample coordinate, phase in cycles) is FP64,
+// which B200 runs at half the FP32 rate; only the interpolation, rotation and accumulation are
+// FP32.  The aperture test repeats the defining expression
+// 4 f#^2 rho^2 <= a^2 with separately rounded FP64 operations so that a voxel/element pair on
+// the edge of the cone is classified exactly as the definition does ("aperture edge").
+#include "das_internal.cuh"
+
+namespace das {
+
+namespace {
+
+constexpr int kQc = 8;          // transmits per pass: 8 complex FP32 accumulators + 8 FP64 tau_tx
+constexpr int kThreads = 128;
+
+// One (mid, slope) table entry of the device layout (das_internal.cuh), widened to FP32.
+struct EntryF { float mid_re, mid_im, slope_re, slope_im; };
+template <typename T> struct Sample;
+template <> struct Sample<float4> {       // IQ fp32
+  static __device__ __forceinline__ EntryF load(const float4* p) { const float4 v = __ldg(p); return {v.x, v.y, v.z, v.w}; }
+};
+template <> struct Sample<uint2> {        // IQ fp16: (half2 mid, half2 slope)
+  static __device__ __forceinline__ EntryF load(const uint2* p) {
+    const uint2 u = __ldg(p);
+    const float2 m = __half22float2(*reinterpret_cast<const __half2*>(&u.x));
+    const float2 s = __half22float2(*reinterpret_cast<const __half2*>(&u.y));
+    return {m.x, m.y, s.x, s.y};
+  }
+};
+template <> struct Sample<float2> {       // RF fp32
+  static __device__ __forceinline__ EntryF load(const float2* p) { const float2 v = __ldg(p); return {v.x, 0.f, v.y, 0.f}; }
+};
+template <> struct Sample<unsigned> {     // RF fp16: half2 (mid, slope)
+  static __device__ __forceinline__ EntryF load(const unsigned* p) {
+    const unsigned u = __ldg(p);
+    const float2 v = __half22float2(*reinterpret_cast<const __half2*>(&u));
+    return {v.x, 0.f, v.y, 0.f};
+  }
+};
+
+template <bool IQ, typename T>
+__global__ void __launch_bounds__(kThreads)
+general_kernel(const Params P, const T* __restrict__ conv, void* __restrict__ out_v) {
+  const long long N = (long long)P.nx * P.ny * P.nz;
+  const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (n >= N) return;
+  const int iz = (int)(n % P.nz);
+  const int iy = (int)((n / P.nz) % P.ny);
+  const int ix = (int)(n / ((long long)P.nz * P.ny));
+  const double px = (double)P.xs[ix], py = (double)P.ys[iy], pz = (double)P.zs[iz];
+  const double inv_c = 1.0 / P.c;
+  const double lim_hi = (double)(P.K - 2);
+  // 4 f#^2, rounded as ((4 f#) f#), the order the definition is evaluated in
+  const double four_f2 = __dmul_rn(__dmul_rn(4.0, P.fnum), P.fnum);
+
+  float tot_re = 0.f, tot_im = 0.f;
+  for (int q0 = 0; q0 < P.Q; q0 += kQc) {
+    double tau_tx[kQc];
+    float acc_re[kQc], acc_im[kQc];
+#pragma unroll
+    for (int j = 0; j < kQc; ++j) {
+      acc_re[j] = 0.f; acc_im[j] = 0.f;
+      const int q = min(q0 + j, P.Q - 1);
+      const TxDev tx = P.tx[q];
+      if (tx.type == DAS_TX_PLANE) {
+        tau_tx[j] = (px * tx.vx + py * tx.vy + pz * tx.vz) * inv_c + tx.t0;
+      } else {
+        const double ax = px - tx.vx, ay = py - tx.vy, az = pz - tx.vz;
+        tau_tx[j] = sqrt(ax * ax + ay * ay + az * az) * inv_c + tx.t0;
+      }
+    }
+    for (int m = 0; m < P.M; ++m) {
+      const float4 e = __ldg(&P.elem[m]);
+      const double dx = px - (double)e.x, dy = py - (double)e.y, dz = pz - (double)e.z;
+      const double dx2 = __dmul_rn(dx, dx), dy2 = __dmul_rn(dy, dy), dz2 = __dmul_rn(dz, dz);
+      const double dd = __dadd_rn(__dadd_rn(dx2, dy2), dz2);
+      if (P.apod) {
+        double a, rho2;
+        if (P.has_dir) {
+          const float4 d = __ldg(&P.edir[m]);
+          a = __dadd_rn(__dadd_rn(__dmul_rn(dx, (double)d.x), __dmul_rn(dy, (double)d.y)),
+                        __dmul_rn(dz, (double)d.z));
+          rho2 = __dadd_rn(dd, -__dmul_rn(a, a));
+        } else {
+          a = dz;
+          rho2 = __dadd_rn(dx2, dy2);
+        }
+        if (!(a > 0.0 && __dmul_rn(four_f2, rho2) <= __dmul_rn(a, a))) continue;
+      }
+      const double tau_rx = sqrt(dd) * inv_c;
+      const T* rowm = conv + (long long)m * P.Q * P.Kp;
+#pragma unroll
+      for (int j = 0; j < kQc; ++j) {
+        if (q0 + j >= P.Q) break;
+        const double tau = tau_tx[j] + tau_rx;
+        const double t = (tau - P.t_start) * P.fs;
+        const double kf = floor(t);
+        if (!(kf >= 0.0 && kf <= lim_hi)) continue;
+        const float ah = (float)(t - kf) - 0.5f;             // y[t] = mid_k + (alpha - 1/2) slope_k
+        const EntryF en = Sample<T>::load(rowm + (long long)(q0 + j) * P.Kp + (kPadLeft + (int)kf));
+        const float s_re = fmaf(ah, en.slope_re, en.mid_re);
+        if (IQ) {
+          const float s_im = fmaf(ah, en.slope_im, en.mid_im);
+          double cyc = P.fc * tau;
+          cyc -= rint(cyc);                        // phase in cycles, reduced to [-1/2, 1/2] in FP64
+          float sn, cs;
+          sincospif(2.0f * (float)cyc, &sn, &cs);
+          acc_re[j] = fmaf(s_re, cs, fmaf(-s_im, sn, acc_re[j]));
+          acc_im[j] = fmaf(s_re, sn, fmaf(s_im, cs, acc_im[j]));
+        } else {
+          acc_re[j] += s_re;
+        }
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < kQc; ++j) { tot_re += acc_re[j]; tot_im += acc_im[j]; }
+  }
+  if (IQ) reinterpret_cast<float2*>(out_v)[n] = make_float2(tot_re, tot_im);
+  else    reinterpret_cast<float*>(out_v)[n] = tot_re;
+}
+
+}  // namespace
+
+cudaError_t launch_general(const Params& P, const void* d_conv, void* d_out, cudaStream_t s) {
+  const long long N = (long long)P.nx * P.ny * P.nz;
+  const unsigned blocks = (unsigned)((N + kThreads - 1) / kThreads);
+  if (P.iq) {
+    if (P.fp16) general_kernel<true, uint2><<<blocks, kThreads, 0, s>>>(P, (const uint2*)d_conv, d_out);
+    else        general_kernel<true, float4><<<blocks, kThreads, 0, s>>>(P, (const float4*)d_conv, d_out);
+  } else {
+    if (P.fp16) general_kernel<false, unsigned><<<blocks, kThreads, 0, s>>>(P, (const unsigned*)d_conv, d_out);
+    else        general_kernel<false, float2><<<blocks, kThreads, 0, s>>>(P, (const float2*)d_conv, d_out);
+  }
+  count_launch();
+  return cudaGetLastError();
+}
+
+}  // namespace das

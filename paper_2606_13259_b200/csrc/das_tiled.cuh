@@ -1,0 +1,415 @@
+// Tiled delay-and-sum kernel for planar arrays (all receivers in one plane z = z_a, normals +z,
+// every voxel in front of that plane) -- the fast path of das_execute.
+//
+// Decomposition:
+//   t_qmn = T_q(n) + e_m(n)                               [samples]
+//     T_q(n) = (tau_tx(q,n) + a_n/c - t_start) fs          a_n = z_n - z_a   per (q, n), FP64
+//     e_m(n) = (|p_n - r_m| - a_n) fs/c
+//            = rho^2 (fs/c) / (a_n + sqrt(rho^2 + a_n^2))                    per (m, n), FP32
+//   phase    exp(j 2 pi fc tau) = Ptx_q(n) * Prx_m(n),
+//     Ptx = exp(j 2 pi (fc t_start + (fc/fs) T_q)),  Prx = exp(j 2 pi (fc/fs) e_m)
+//   x_n = sum_q Ptx_q(n) * [ sum_m w_mn Prx_m(n) y_qm[t_qmn] ]
+// The part common to all receivers of a voxel (whose rounding error would add coherently) is
+// FP64 and amortised over M; the per-receiver excess path e_m is small (<= ~0.12 a fs/c inside
+// an f/1 cone), so FP32 keeps ~1e-6 samples on it.
+//
+// Work split inside a CTA (one CTA = one voxel tile at a time, persistent over a static,
+// work-sorted tile list):
+//   * ONE producer warp walks the tile's active-receiver list (built by the plan).  For each
+//     receiver m it issues, per transmit q of the current chunk, one TMA bulk copy
+//     (cp.async.bulk global -> shared, completion counted on an mbarrier) of the W table entries
+//     [k0, k0 + W), k0 = K0tile_q + E0_m, of row (m, q) of the converted channel data.  The
+//     entries are already (mid, slope) pairs with zeros outside the valid sample range
+//     (das_internal.cuh), so staging is a pure copy: no producer arithmetic, no bounds tests.
+//   * consumer threads own one voxel each (a warp = 8 x 4 lateral voxels at one depth, so all
+//     lanes read nearly the same shared-memory words: broadcast), keep QC complex accumulators
+//     and QC reduced transmit delays in registers, and run the (m outer, q inner) loop:
+//       ts = Tf_q + e'          u = ts + MAGIC (rounds to the entry index)   al = ts - (u - MAGIC)
+//       (mid, slope) = table[u]             s = mid + al * slope            acc_q += Prx * s
+//     Index arithmetic and the complex multiply-accumulate are issued as packed FP32x2
+//     instructions (FADD2 / FFMA2, new on sm_100) over pairs of transmits.
+//   * stages travel through an mbarrier ring (full: expect_tx + TMA complete_tx; empty: one
+//     arrive per consumer warp), so L2 latency is hidden behind the consumers' arithmetic.
+#pragma once
+
+#include "das_internal.cuh"
+
+namespace das {
+
+constexpr int kStages = 8;
+constexpr int kLaneX = 8, kLaneY = 4;          // a consumer warp covers 8 x 4 lateral voxels
+constexpr int kWX = 1, kWY = 2, kWZ = 4;       // consumer warps per tile: tile = 8 x 8 x 4 voxels
+constexpr int kConsumerWarps = kWX * kWY * kWZ;
+constexpr int kTiledThreads = (kConsumerWarps + 1) * 32;
+constexpr float kMagic = 12582912.0f;           // 1.5 * 2^23: adding it rounds to an integer
+constexpr unsigned kMagicBits = 0x4B400000u;
+constexpr float kBand = 4e-6f;                  // relative guard band of the FP32 aperture test
+
+enum Mode { kIQ32 = 0, kIQ16 = 1, kRF32 = 2, kRF16 = 3 };
+template <int MODE> struct ModeTraits;
+template <> struct ModeTraits<kIQ32> { static constexpr bool iq = true;  static constexpr int eb = 16; };
+template <> struct ModeTraits<kIQ16> { static constexpr bool iq = true;  static constexpr int eb = 8; };
+template <> struct ModeTraits<kRF32> { static constexpr bool iq = false; static constexpr int eb = 8; };
+template <> struct ModeTraits<kRF16> { static constexpr bool iq = false; static constexpr int eb = 4; };
+__host__ __device__ inline int entry_bytes(int iq, int fp16) { return (iq ? 2 : 1) * 2 * (fp16 ? 2 : 4); }
+
+struct TileDesc {       // one voxel tile
+  int ix0, iy0, iz0;    // origin (voxel indices)
+  int list_off;         // offset into the receiver list
+  int list_cnt;         // number of (potentially) active receivers
+};
+
+struct TiledDev {
+  int n_tiles;
+  int n_chunks;               // ceil(Q / QC)
+  const TileDesc* tiles;      // [n_tiles], sorted by decreasing work
+  const int* k0tile;          // [n_tiles][Q]   window origin per transmit (multiple of 16/eb)
+  const unsigned* list;       // receiver lists: m | (E0 << 16), E0 a multiple of 16/eb
+  double z_array;             // z_a
+  double kappa;               // fs / c
+  double ratio;               // fc / fs
+  double phase0;              // frac(fc * t_start), cycles
+  float four_f2;              // 4 f#^2
+};
+
+// ---- PTX helpers ---------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) {
+  return static_cast<unsigned>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+// TMA bulk copy global -> this CTA's shared memory, completion (bytes) counted on an mbarrier
+__device__ __forceinline__ void tma_bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+template <int OFF> __device__ __forceinline__ float4 lds128(unsigned addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4+%5];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr), "n"(OFF));
+  return v;
+}
+template <int OFF> __device__ __forceinline__ uint2 lds64(unsigned addr) {
+  uint2 v;
+  asm volatile("ld.shared.v2.b32 {%0,%1}, [%2+%3];" : "=r"(v.x), "=r"(v.y) : "r"(addr), "n"(OFF));
+  return v;
+}
+template <int OFF> __device__ __forceinline__ unsigned lds32(unsigned addr) {
+  unsigned v;
+  asm volatile("ld.shared.b32 %0, [%1+%2];" : "=r"(v) : "r"(addr), "n"(OFF));
+  return v;
+}
+__device__ __forceinline__ float rsqrt_approx(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rcp_approx(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float sin_approx(float x) { float r; asm("sin.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float cos_approx(float x) { float r; asm("cos.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
+template <int QC, int W, int MODE>
+struct alignas(128) TiledSmem {
+  unsigned char tab[kStages][QC * W * ModeTraits<MODE>::eb];
+  float4 meta[kStages];                 // (ex, ey, E0, unused) of the staged receiver
+  unsigned long long full[kStages];
+  unsigned long long empty[kStages];
+};
+
+// exact (definition-order, FP64) aperture test for pairs inside the FP32 guard band
+static __device__ __noinline__ bool aperture_exact(float x, float y, float ex, float ey, double a, double fnum) {
+  const double dx = (double)x - (double)ex, dy = (double)y - (double)ey;
+  const double rho2 = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
+  const double four_f2 = __dmul_rn(__dmul_rn(4.0, fnum), fnum);
+  return __dmul_rn(four_f2, rho2) <= __dmul_rn(a, a);
+}
+
+__device__ __forceinline__ double tx_delay(const TxDev& tx, double x, double y, double z, double c) {
+  if (tx.type == DAS_TX_PLANE) return (x * tx.vx + y * tx.vy + z * tx.vz) / c + tx.t0;
+  const double bx = x - tx.vx, by = y - tx.vy, bz = z - tx.vz;
+  return sqrt(bx * bx + by * by + bz * bz) / c + tx.t0;
+}
+
+// One interpolated sample per transmit of the pair (j, j+1): returns s (re, im) for each.
+template <int MODE, int OFF0, int OFF1>
+__device__ __forceinline__ void gather_pair(unsigned a0, unsigned a1, float2 al, float2& sre, float2& sim) {
+  if constexpr (MODE == kIQ32) {
+    const float4 v0 = lds128<OFF0>(a0);
+    const float4 v1 = lds128<OFF1>(a1);
+    sre = make_float2(fmaf(al.x, v0.z, v0.x), fmaf(al.y, v1.z, v1.x));
+    sim = make_float2(fmaf(al.x, v0.w, v0.y), fmaf(al.y, v1.w, v1.y));
+  } else if constexpr (MODE == kIQ16) {
+    const uint2 v0 = lds64<OFF0>(a0);
+    const uint2 v1 = lds64<OFF1>(a1);
+    const __half2 alh = __floats2half2_rn(al.x, al.y);
+    const __half2 s0 = __hfma2(__low2half2(alh), *reinterpret_cast<const __half2*>(&v0.y), *reinterpret_cast<const __half2*>(&v0.x));
+    const __half2 s1 = __hfma2(__high2half2(alh), *reinterpret_cast<const __half2*>(&v1.y), *reinterpret_cast<const __half2*>(&v1.x));
+    sre = make_float2(__low2float(s0), __low2float(s1));
+    sim = make_float2(__high2float(s0), __high2float(s1));
+  } else if constexpr (MODE == kRF32) {
+    const uint2 v0 = lds64<OFF0>(a0);
+    const uint2 v1 = lds64<OFF1>(a1);
+    sre = make_float2(fmaf(al.x, __uint_as_float(v0.y), __uint_as_float(v0.x)),
+                      fmaf(al.y, __uint_as_float(v1.y), __uint_as_float(v1.x)));
+    sim = make_float2(0.f, 0.f);
+  } else {
+    const unsigned w0 = lds32<OFF0>(a0);
+    const unsigned w1 = lds32<OFF1>(a1);
+    const float2 f0 = __half22float2(*reinterpret_cast<const __half2*>(&w0));
+    const float2 f1 = __half22float2(*reinterpret_cast<const __half2*>(&w1));
+    sre = make_float2(fmaf(al.x, f0.y, f0.x), fmaf(al.y, f1.y, f1.x));
+    sim = make_float2(0.f, 0.f);
+  }
+}
+
+template <int QC, int W, int MODE>
+__global__ void __launch_bounds__(kTiledThreads, 2)
+tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict__ conv, void* __restrict__ out_v) {
+  constexpr bool IQ = ModeTraits<MODE>::iq;
+  constexpr int EB = ModeTraits<MODE>::eb;
+  constexpr int ESH = (EB == 16) ? 4 : (EB == 8) ? 3 : 2;
+  constexpr int QP = (QC + 1) / 2;                   // transmit pairs per chunk
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  TiledSmem<QC, W, MODE>& sm = *reinterpret_cast<TiledSmem<QC, W, MODE>*>(smem_raw);
+
+  const int tid = threadIdx.x;
+  const int warp = tid >> 5, lane = tid & 31;
+  const unsigned full0 = smem_u32(&sm.full[0]), empty0 = smem_u32(&sm.empty[0]);
+  if (tid == 0) {
+    for (int s = 0; s < kStages; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, kConsumerWarps); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  unsigned seq = 0;          // stages produced / consumed so far by this CTA (same count on both sides)
+
+  if (warp == kConsumerWarps) {
+    // =============================== PRODUCER (TMA) =========================================
+    const unsigned tab0 = smem_u32(&sm.tab[0][0]);
+    for (int tile_i = blockIdx.x; tile_i < tp.n_tiles; tile_i += gridDim.x) {
+      const TileDesc td = tp.tiles[tile_i];
+      for (int ch = 0; ch < tp.n_chunks; ++ch) {
+        const int q = ch * QC + lane;
+        const bool qok = lane < QC && q < P.Q;
+        const int k0 = qok ? __ldg(&tp.k0tile[(long long)tile_i * P.Q + q]) : 0;
+        const int nq = min(QC, P.Q - ch * QC);
+        for (int li = 0; li < td.list_cnt; ++li, ++seq) {
+          const unsigned slot = seq % kStages;
+          const unsigned ent = __ldg(&tp.list[td.list_off + li]);
+          const int m = (int)(ent & 0xFFFFu);
+          const int e0 = (int)(ent >> 16);
+          const float4 el = __ldg(&P.elem[m]);
+          mbar_wait(empty0 + 8 * slot, ((seq / kStages) & 1u) ^ 1u);
+          if (lane == 0) {
+            sm.meta[slot] = make_float4(el.x, el.y, (float)e0, 0.f);
+            mbar_arrive_expect_tx(full0 + 8 * slot, (unsigned)(nq * W * EB));
+          }
+          __syncwarp();
+          if (qok) {
+            int i0 = kPadLeft + k0 + e0;                  // first table entry of the window
+            i0 = max(0, min(i0, P.Kp - W));               // clamped windows lie entirely in a zero pad
+            const unsigned char* src = conv + (((long long)m * P.Q + q) * P.Kp + i0) * EB;
+            tma_bulk_g2s(tab0 + slot * (QC * W * EB) + lane * (W * EB), src, W * EB, full0 + 8 * slot);
+          }
+        }
+      }
+    }
+    return;
+  }
+
+  // ================================= CONSUMERS ==============================================
+  const int wz = warp / (kWX * kWY), wy = (warp / kWX) % kWY, wx = warp % kWX;
+  const int lx = lane % kLaneX, ly = lane / kLaneX;
+  const float kappa = (float)tp.kappa;
+  const float ratio = (float)tp.ratio;
+  // table address of entry index bits: (bits(u) << ESH) + base_adj, where bits(u) still holds
+  // the float exponent pattern of MAGIC; base_adj removes it (mod 2^32)
+  unsigned base_adj = smem_u32(&sm.tab[0][0]) - (kMagicBits << ESH);
+  asm volatile("mov.b32 %0, %0;" : "+r"(base_adj));     // opaque: keeps (bits << ESH) + base one LEA
+
+  for (int tile_i = blockIdx.x; tile_i < tp.n_tiles; tile_i += gridDim.x) {
+    const TileDesc td = tp.tiles[tile_i];
+    const int ix = td.ix0 + wx * kLaneX + lx;
+    const int iy = td.iy0 + wy * kLaneY + ly;
+    const int iz = td.iz0 + wz;
+    const bool in_grid = ix < P.nx && iy < P.ny && iz < P.nz;
+    const float x = P.xs[min(ix, P.nx - 1)], y = P.ys[min(iy, P.ny - 1)], z = P.zs[min(iz, P.nz - 1)];
+    const double a_d = (double)z - tp.z_array;
+    const float a = (float)a_d;
+    const float a2 = a * a;
+    float out_re = 0.f, out_im = 0.f;
+
+    for (int ch = 0; ch < tp.n_chunks; ++ch) {
+      const int q0 = ch * QC;
+      // ---- per-(q, n) part in FP64: reduced transmit delay -------------------------------
+      float2 Tf[QP];
+      float2 accR[QP], accI[QP];          // (acc_j, acc_j+1) real and imaginary parts
+#pragma unroll
+      for (int jp = 0; jp < QP; ++jp) {
+        float tf[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int q = min(q0 + 2 * jp + h, P.Q - 1);
+          const double T = (tx_delay(P.tx[q], x, y, z, P.c) + a_d / P.c - P.t_start) * P.fs;
+          const int k0 = __ldg(&tp.k0tile[(long long)tile_i * P.Q + q]);
+          tf[h] = (float)(T - (double)k0 - 0.5);
+        }
+        Tf[jp] = make_float2(tf[0], tf[1]);
+        accR[jp] = make_float2(0.f, 0.f);
+        accI[jp] = make_float2(0.f, 0.f);
+      }
+
+      // ---- receiver loop ---------------------------------------------------------------
+      for (int li = 0; li < td.list_cnt; ++li, ++seq) {
+        const unsigned slot = seq % kStages;
+        mbar_wait(full0 + 8 * slot, (seq / kStages) & 1u);
+        const float4 meta = sm.meta[slot];
+        const float dx = x - meta.x, dy = y - meta.y;
+        const float rho2 = fmaf(dx, dx, dy * dy);
+        bool act = in_grid;
+        if (P.apod) {
+          const float lhs = tp.four_f2 * rho2;
+          bool in = lhs <= a2;
+          if (fabsf(lhs - a2) <= kBand * a2) in = aperture_exact(x, y, meta.x, meta.y, a_d, P.fnum);
+          act = act && in;
+        }
+        if (act) {
+          const float s2 = rho2 + a2;
+          const float d = s2 * rsqrt_approx(s2);
+          const float e = (rho2 * kappa) * rcp_approx(a + d);
+          const float ep = e - meta.z;
+          float pr = 1.f, pi = 0.f;
+          if (IQ) {
+            float cyc = ratio * e;
+            cyc -= rintf(cyc);
+            const float ang = 6.283185307179586f * cyc;
+            pr = cos_approx(ang);
+            pi = sin_approx(ang);
+          }
+          const float magic = kMagic + (float)(slot * (QC * W));
+          const float2 ep2 = make_float2(ep, ep), mg2 = make_float2(magic, magic), nmg2 = make_float2(-magic, -magic);
+          const float2 neg1 = make_float2(-1.f, -1.f);
+          const float2 prr = make_float2(pr, pr), pii = make_float2(pi, pi), npi = make_float2(-pi, -pi);
+#pragma unroll
+          for (int jp = 0; jp < QP; ++jp) {
+            const float2 ts = __fadd2_rn(Tf[jp], ep2);
+            const float2 u = __fadd2_rn(ts, mg2);
+            const float2 kf = __fadd2_rn(u, nmg2);
+            const float2 al = __ffma2_rn(kf, neg1, ts);
+            const unsigned a0 = (__float_as_uint(u.x) << ESH) + base_adj;
+            const unsigned a1 = (__float_as_uint(u.y) << ESH) + base_adj;
+            float2 sre, sim;
+            constexpr int kRow = W * EB;
+            // immediates: row offsets of transmit 2 jp and 2 jp + 1 inside a stage
+            switch (jp) {
+#define DAS_CASE(JP) case JP: gather_pair<MODE, (2 * JP) * kRow, ((2 * JP + 1) % (QC > 1 ? QC : 1)) * kRow>(a0, a1, al, sre, sim); break;
+              DAS_CASE(0) DAS_CASE(1) DAS_CASE(2) DAS_CASE(3) DAS_CASE(4) DAS_CASE(5) DAS_CASE(6) DAS_CASE(7)
+#undef DAS_CASE
+              default: sre = sim = make_float2(0.f, 0.f);
+            }
+            if (IQ) {
+              accR[jp] = __ffma2_rn(sre, prr, accR[jp]);
+              accR[jp] = __ffma2_rn(sim, npi, accR[jp]);
+              accI[jp] = __ffma2_rn(sre, pii, accI[jp]);
+              accI[jp] = __ffma2_rn(sim, prr, accI[jp]);
+            } else {
+              accR[jp] = __fadd2_rn(accR[jp], sre);
+            }
+          }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty0 + 8 * slot);
+      }
+
+      // ---- fold this chunk: x += sum_q Ptx_q * acc_q ---------------------------------------
+#pragma unroll
+      for (int jp = 0; jp < QP; ++jp) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int q = q0 + 2 * jp + h;
+          if (2 * jp + h < QC && q < P.Q) {
+            const float are = h ? accR[jp].y : accR[jp].x;
+            const float aim = h ? accI[jp].y : accI[jp].x;
+            if (IQ) {
+              const double T = (tx_delay(P.tx[q], x, y, z, P.c) + a_d / P.c - P.t_start) * P.fs;
+              double cyc = tp.phase0 + tp.ratio * T;
+              cyc -= rint(cyc);
+              float sn, cs;
+              sincospif(2.0f * (float)cyc, &sn, &cs);
+              out_re = fmaf(are, cs, fmaf(-aim, sn, out_re));
+              out_im = fmaf(are, sn, fmaf(aim, cs, out_im));
+            } else {
+              out_re += are;
+            }
+          }
+        }
+      }
+    }
+    if (in_grid) {
+      const long long n = ((long long)ix * P.ny + iy) * P.nz + iz;
+      if (IQ) reinterpret_cast<float2*>(out_v)[n] = make_float2(out_re, out_im);
+      else    reinterpret_cast<float*>(out_v)[n] = out_re;
+    }
+  }
+}
+
+// ---- per-mode launcher, instantiated in das_tiled_inst_*.cu ----------------------------------
+template <int QC, int W, int MODE>
+cudaError_t launch_tiled_inst(const TiledDev& tp, const Params& P, const void* conv, void* out, int grid, cudaStream_t s) {
+  auto k = tiled_kernel<QC, W, MODE>;
+  const size_t smem = sizeof(TiledSmem<QC, W, MODE>);
+  static bool configured = false;        // per instantiation
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  k<<<grid, kTiledThreads, smem, s>>>(tp, P, static_cast<const unsigned char*>(conv), out);
+  return cudaGetLastError();
+}
+
+template <int QC, int MODE>
+cudaError_t launch_tiled_w(int W, const TiledDev& tp, const Params& P, const void* conv, void* out, int grid, cudaStream_t s) {
+  switch (W) {
+    case 16: return launch_tiled_inst<QC, 16, MODE>(tp, P, conv, out, grid, s);
+    case 20: return launch_tiled_inst<QC, 20, MODE>(tp, P, conv, out, grid, s);
+    case 24: return launch_tiled_inst<QC, 24, MODE>(tp, P, conv, out, grid, s);
+    case 32: return launch_tiled_inst<QC, 32, MODE>(tp, P, conv, out, grid, s);
+    case 48: return launch_tiled_inst<QC, 48, MODE>(tp, P, conv, out, grid, s);
+    case 64: return launch_tiled_inst<QC, 64, MODE>(tp, P, conv, out, grid, s);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+template <int MODE>
+cudaError_t launch_tiled_mode(int QC, int W, const TiledDev& tp, const Params& P, const void* conv, void* out, int grid, cudaStream_t s) {
+  switch (QC) {
+    case 1: return launch_tiled_w<1, MODE>(W, tp, P, conv, out, grid, s);
+    case 2: return launch_tiled_w<2, MODE>(W, tp, P, conv, out, grid, s);
+    case 4: return launch_tiled_w<4, MODE>(W, tp, P, conv, out, grid, s);
+    case 8: return launch_tiled_w<8, MODE>(W, tp, P, conv, out, grid, s);
+    case 16: return launch_tiled_w<16, MODE>(W, tp, P, conv, out, grid, s);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+// defined one per TU
+cudaError_t launch_tiled_iq32(int QC, int W, const TiledDev&, const Params&, const void*, void*, int grid, cudaStream_t);
+cudaError_t launch_tiled_iq16(int QC, int W, const TiledDev&, const Params&, const void*, void*, int grid, cudaStream_t);
+cudaError_t launch_tiled_rf32(int QC, int W, const TiledDev&, const Params&, const void*, void*, int grid, cudaStream_t);
+cudaError_t launch_tiled_rf16(int QC, int W, const TiledDev&, const Params&, const void*, void*, int grid, cudaStream_t);
+
+constexpr int kWindows[] = {16, 20, 24, 32, 48, 64};
+
+}  // namespace das
