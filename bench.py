@@ -1,0 +1,409 @@
+#!/usr/bin/env python
+"""bench.py -- volumetric delay-and-sum throughput on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl cuda|reference]
+                    [--config 3] [--storage fp16|fp32] [--algo auto|general|tiled]
+
+One "step" is one pass of the whole hot path over one frame of
+synthetic channel data already resident in HBM: das_convert (layout transform + cast) followed
+by das_execute (delays, aperture, gather, interpolation, rotation, accumulation, store), both
+through the C ABI of libdas_b200.so.  The default workload is BASELINE.json configs[2], the
+headline the metric is quoted on: 128^3 voxels x 1024 elements x 16 diverging-wave transmits,
+1024 IQ samples per trace, fp16 storage.
+
+Printed: ONE JSON line (rank 0).  Keys beyond the base contract:
+  roofline      the dominant kernel (das_execute's tiled kernel) against the FP32 ALU roofline
+  cpu_baseline  the CPU oracle (oracle/, as it stands) timed on this box's host cores on a
+                bounded voxel sample of the same workload
+  e2e           the same metric through das_beamform_host with pinned HOST buffers (H2D of the
+                raw frame and D2H of the volume inside the timed region)
+
+Multi-GPU: the path does not shard inside one volume (north_star: one GPU); --gpus N runs N
+independent replicas, one process per GPU, no data-path collective ("replicas only").
+torch.distributed is used for the barrier and the max-over-ranks of the device time only.
+
+--impl reference times the CPU oracle itself (this tier's reference arm): each step is a bounded
+voxel sample of the same workload.  It is the only other place the oracle may run.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "volumes/s at 128^3 vox, 1024 el, 16 tx"
+UNIT = "volumes/s"
+
+# Definition flops per unit of algorithmic work:
+#   per entered (q, m, n) term   IQ: 17 (delay add 1, index/fraction split 2, lerp 6, complex MAC 8)
+#                                RF:  8 (add 1, split 2, lerp 3, weighted add 2)
+#   per active (m, n) pair       28 (2 sub, 3 FMA, sqrt, reciprocal, compare, rx phase sincos)
+FLOPS_PER_TERM = {0: 17.0, 1: 8.0}
+FLOPS_PER_PAIR = 28.0
+FP32_LANES_PER_SM = 128          # B200_PROFILING.md / B300_MICROARCH.md: 4 SMSP x 32 lanes
+N_SM = 148
+
+# dram__bytes_read.sum + dram__bytes_write.sum of the tiled kernel, per launch, from the
+# `ncu --set full` capture summarised in profiles/ (bytes); keyed by (config, storage).
+NCU_TRAFFIC_BYTES = {
+    (3, "fp16"): 57.4e6,         # profiles/r1_tiled_iq16_full.md
+}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4],
+                    help="BASELINE.json config number (3 = headline, the metric's workload)")
+    ap.add_argument("--storage", choices=["fp16", "fp32"], default="fp16")
+    ap.add_argument("--algo", choices=["auto", "general", "tiled"], default="auto")
+    ap.add_argument("--frames", type=int, default=4,
+                    help="distinct raw frames rotated through the timed steps (inputs > L2)")
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0,
+                    help="target CPU time of the cpu_baseline oracle sample (0 = skip)")
+    return ap.parse_args()
+
+
+def dist_env():
+    return (int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")),
+            int(os.environ.get("WORLD_SIZE", "1")))
+
+
+def workload_name(w, storage):
+    nx, ny, nz = w.grid_shape
+    kind = "IQ" if w.data_kind == 0 else "RF"
+    return (f"config{w.seed - 20260612} {w.name}: {nx}x{ny}x{nz} voxels, {w.n_elem} elements, "
+            f"{w.n_tx} transmits, K={w.n_samples} {kind} samples, {storage} storage, f/1 boxcar")
+
+
+# ------------------------------------------------------------------------------------------
+# clocks: sample NVML while the timed region runs
+# ------------------------------------------------------------------------------------------
+
+class ClockSampler:
+    """Polls SM clock and throttle reasons of one GPU from a background thread (NVML)."""
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown",
+               0x4: "sw_power_cap", 0x80: "hw_power_brake_slowdown"}
+
+    def __init__(self, index: int, period_s: float = 0.01):
+        self.samples, self.reasons, self.power = [], set(), []
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thread = None
+        self._period = period_s
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:                      # NVML missing: report that, never fake clocks
+            self._nv, self._err = None, repr(e)
+
+    def _run(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                for bit, name in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self._h) / 1000.0)
+            except Exception:
+                pass
+            self._stop.wait(self._period)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+
+    def summary(self):
+        if self._nv is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "error": self._err}
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples),
+                "power_w_max": max(self.power) if self.power else None}
+
+
+# ------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline of the cuda arm; the whole of --impl reference)
+# ------------------------------------------------------------------------------------------
+
+def oracle_sample(w, n_vox, seed):
+    """Time the oracle (as it stands) on ``n_vox`` voxels drawn uniformly from the volume.
+    Uniform sampling keeps the depth mix, hence the active-aperture mix, of the full volume."""
+    import oracle
+    rng = np.random.default_rng(seed)
+    vox = rng.integers(0, w.n_voxels, size=int(n_vox)).astype(np.int64)
+    t0 = time.perf_counter()
+    oracle.das(w, voxels=vox)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(w, target_s):
+    """Bounded sample of the workload on the host cores -> volumes/s (extrapolated linearly in
+    the voxel count, which is exact for this embarrassingly parallel sum)."""
+    import oracle
+    threads = oracle.threads()
+    probe = min(512, w.n_voxels)
+    oracle_sample(w, 64, 1)                                   # load the library, warm caches
+    dt = oracle_sample(w, probe, 2)
+    n = int(min(max(probe, target_s / max(dt, 1e-9) * probe), w.n_voxels, 200000))
+    dt = oracle_sample(w, n, 3)
+    return {"value": (n / dt) / w.n_voxels, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": f"{n} of {w.n_voxels} voxels drawn uniformly (all {w.n_elem} elements x "
+                      f"{w.n_tx} transmits each), {dt:.1f} s of oracle time, extrapolated by voxel count",
+            "seconds": dt}
+
+
+def run_reference(args):
+    """--impl reference: the oracle IS the reference arm for this tier.  Rank 0 only."""
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    import workloads as wl
+    import oracle
+    w = wl.config(args.config)
+    threads = oracle.threads()
+    oracle_sample(w, 64, 1)
+    probe = oracle_sample(w, 256, 2)
+    # size each step so the whole run (warmup + steps) stays within ~2 minutes
+    budget = 120.0 / max(args.steps + args.warmup, 1)
+    n = int(min(max(64, budget / max(probe, 1e-9) * 256), w.n_voxels, 100000))
+    for i in range(args.warmup):
+        oracle_sample(w, n, 10 + i)
+    times = [oracle_sample(w, n, 100 + i) for i in range(args.steps)]
+    total = float(sum(times))
+    value = (n * args.steps / total) / w.n_voxels
+    sample = (f"each step = {n} of {w.n_voxels} voxels drawn uniformly (all elements x transmits), "
+              f"extrapolated by voxel count")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": workload_name(w, args.storage),
+                       "note": "the oracle reads the raw float32 channel data (no storage cast)"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------
+# CUDA arm
+# ------------------------------------------------------------------------------------------
+
+BAD_REASONS = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"}
+
+
+def make_frames(w, n_frames):
+    """Frame 0 is the config's seeded channel data; frames f > 0 add an independent seeded
+    noise realisation (sigma 0.01) so that every timed step reads different bytes.  The rotation
+    through > 126 MB of distinct input is what defeats L2 reuse between steps."""
+    frames = [w.y]
+    iq = w.data_kind == 0
+    for f in range(1, n_frames):
+        rng = np.random.default_rng(w.seed + 7919 * f)
+        if iq:
+            sd = 0.01 / np.sqrt(2.0)
+            n = (rng.normal(0.0, sd, w.y.shape) + 1j * rng.normal(0.0, sd, w.y.shape)).astype(np.complex64)
+        else:
+            n = rng.normal(0.0, 0.01, w.y.shape).astype(np.float32)
+        frames.append(w.y + n)
+    return frames
+
+
+def fp32_peak_tflops(sampler_max_mhz):
+    """148 SMs x 128 FP32 lanes x 2 flop (FMA) x max SM clock.  The clock is the driver-measured
+    sm_max_mhz of MEASURED_PEAKS.json when present, else NVML's max SM clock, else 1965 MHz."""
+    mhz, src = None, None
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            mhz = float(json.load(f)["sm_max_mhz"])
+            src = "MEASURED_PEAKS.json sm_max_mhz"
+    except Exception:
+        pass
+    if mhz is None and sampler_max_mhz:
+        mhz, src = float(sampler_max_mhz), "NVML max SM clock"
+    if mhz is None:
+        mhz, src = 1965.0, "B200_PROFILING.md nominal 1965 MHz (fallback)"
+    return N_SM * FP32_LANES_PER_SM * 2 * mhz * 1e6 / 1e12, f"148 SM x 128 lanes x 2 flop x {mhz:.0f} MHz ({src})"
+
+
+def run_cuda(args):
+    import torch
+    import workloads as wl
+    import paper_2606_13259_b200 as das
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the DAS product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    else:
+        dist = None
+    das.load()                                   # raises if libdas_b200.so is missing
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if dist is None:
+            return float(x)
+        t = torch.tensor([float(x)], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    w = wl.config(args.config)
+    storage = das.STORE_FP16 if args.storage == "fp16" else das.STORE_FP32
+    algo = {"auto": das.ALGO_AUTO, "general": das.ALGO_GENERAL, "tiled": das.ALGO_TILED}[args.algo]
+    plan = das.Plan.from_workload(w, storage=storage, algo=algo, device=local_rank)
+    algo_used = {das.ALGO_GENERAL: "general", das.ALGO_TILED: "tiled"}[plan.algo]
+    n_pairs, n_terms = plan.count_work()
+
+    frames_np = make_frames(w, max(1, args.frames))
+    raw = [torch.from_numpy(np.ascontiguousarray(f)).to(dev) for f in frames_np]
+    conv = torch.empty(plan.converted_bytes, dtype=torch.uint8, device=dev)
+    out = torch.empty(w.grid_shape, dtype=torch.complex64 if w.data_kind == 0 else torch.float32, device=dev)
+    stream = torch.cuda.Stream(device=dev)
+    sp = stream.cuda_stream
+
+    def step(i, evs=None):
+        r = raw[i % len(raw)]
+        if evs is not None:
+            evs[0].record(stream)
+        plan.convert(r.data_ptr(), conv.data_ptr(), 1.0, sp)
+        if evs is not None:
+            evs[1].record(stream)
+        plan.execute(conv.data_ptr(), out.data_ptr(), sp)
+        if evs is not None:
+            evs[2].record(stream)
+
+    def measure():
+        for i in range(args.warmup):
+            step(i)
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+        t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        n0 = das.launch_count()
+        with ClockSampler(local_rank) as cs:
+            t_beg.record(stream)
+            for i in range(args.steps):
+                step(args.warmup + i, evs[i])
+            t_end.record(stream)
+            stream.synchronize()
+        launches = das.launch_count() - n0
+        barrier()
+        total_ms = max_over_ranks(t_beg.elapsed_time(t_end))
+        conv_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+        exec_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+        return total_ms, conv_ms, exec_ms, launches, cs.summary()
+
+    total_ms, conv_ms, exec_ms, launches, clocks = measure()
+    remeasured = False
+    if BAD_REASONS & set(clocks.get("reasons", [])):
+        remeasured = True
+        time.sleep(2.0)
+        total_ms, conv_ms, exec_ms, launches, clocks = measure()
+    clocks["remeasured"] = remeasured
+
+    # ---- end to end through das_beamform_host: pinned host buffers, H2D + D2H inside the timing
+    h_raw = [torch.from_numpy(np.ascontiguousarray(f)).pin_memory() for f in frames_np]
+    h_out = torch.empty(w.grid_shape, dtype=out.dtype).pin_memory()
+    plan.beamform_host(h_raw[0].data_ptr(), h_out.data_ptr(), sp)          # allocates the staging
+    e_steps = max(1, args.e2e_steps)
+    e_beg, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e_beg.record(stream)
+    for i in range(e_steps):
+        plan.beamform_host(h_raw[i % len(h_raw)].data_ptr(), h_out.data_ptr(), sp)
+    e_end.record(stream)
+    stream.synchronize()
+    barrier()
+    e2e_ms = max_over_ranks(e_beg.elapsed_time(e_end))
+    checksum = float(h_out.abs().max())                                   # the D2H result is read
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    value = world * args.steps / (total_ms * 1e-3)
+    flops = FLOPS_PER_TERM[w.data_kind] * n_terms + FLOPS_PER_PAIR * n_pairs
+    peak, peak_how = fp32_peak_tflops(clocks.get("sm_max_mhz"))
+    achieved = flops / (exec_ms * 1e-3) / 1e12
+    traffic = NCU_TRAFFIC_BYTES.get((args.config, args.storage)) if algo_used == "tiled" else None
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(w, args.storage), "kernel": algo_used,
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": f"{len(raw)} distinct raw frames rotated ({sum(r.nbytes for r in raw) / 1e6:.0f} MB + "
+                         f"{conv.nbytes / 1e6:.0f} MB converted buffer rewritten every step) > 126 MB L2",
+                   "step": "das_convert + das_execute on device-resident input"},
+        "accumulations_per_s": {"nominal": w.nominal_accumulations * value, "entered": n_terms * value,
+                                "nominal_per_volume": w.nominal_accumulations, "entered_per_volume": n_terms,
+                                "active_pairs_per_volume": n_pairs},
+        "kernels_ms": {"das_convert": conv_ms, "das_execute": exec_ms},
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                     "frac": achieved / peak, "traffic": traffic,
+                     "kernel": f"das_execute ({algo_used} kernel)", "kernel_ms": exec_ms,
+                     "share_of_step": exec_ms / (total_ms / args.steps),
+                     "flops_per_launch": flops,
+                     "flops_model": f"{FLOPS_PER_TERM[w.data_kind]:.0f} x entered terms + {FLOPS_PER_PAIR:.0f} x active (m,n) pairs (DESIGN.md)",
+                     "peak_how": peak_how + ", derived (of derived FP32 peak, not of a measured one)"},
+        "e2e": {"value": world * e_steps / (e2e_ms * 1e-3), "unit": UNIT,
+                "h2d_bytes_per_step": int(plan.raw_bytes), "d2h_bytes_per_step": int(plan.output_bytes),
+                "ms_per_step": e2e_ms / e_steps, "steps": e_steps, "api": "das_beamform_host, pinned host buffers",
+                "checksum_max_abs": checksum},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+    }
+    if world == 1 and args.cpu_seconds > 0:
+        line["cpu_baseline"] = cpu_baseline(w, args.cpu_seconds)
+    else:
+        line["cpu_baseline"] = None
+    print(json.dumps(line), flush=True)
+    plan.destroy()
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -121,6 +121,14 @@ das_status_t das_execute(const das_plan_t* plan, const void* d_conv, void* d_out
  * copy bandwidth h_raw / h_out should be page-locked. */
 das_status_t das_beamform_host(das_plan_t* plan, const void* h_raw, void* h_out, void* stream);
 
+/* Work accounting (used by the bench's roofline; not part of the hot path).  Runs a counting
+ * kernel on the plan's device and SYNCHRONISES.  On success
+ *   *n_pairs = number of (m, n) receiver/voxel pairs with non-zero receive weight w_rx
+ *   *n_terms = number of (q, m, n) terms that enter Eq. 2: non-zero weight and 0 <= k <= K-2
+ * both classified exactly as das_execute classifies them.  Host pointers. */
+das_status_t das_plan_count_work(const das_plan_t* plan, unsigned long long* n_pairs,
+                                 unsigned long long* n_terms);
+
 const char* das_status_string(das_status_t s);
 const char* das_last_error(void);        /* thread-local, never NULL */
 

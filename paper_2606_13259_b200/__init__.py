@@ -31,7 +31,7 @@ ALGO_AUTO, ALGO_GENERAL, ALGO_TILED = 0, 1, 2
 # every symbol include/das.h declares (checked against the header by tests/test_abi.py)
 EXPORTS = ("das_plan_create", "das_plan_destroy", "das_raw_bytes", "das_converted_bytes",
            "das_output_bytes", "das_plan_algo", "das_convert", "das_execute", "das_beamform_host",
-           "das_status_string", "das_last_error", "das_launch_count")
+           "das_plan_count_work", "das_status_string", "das_last_error", "das_launch_count")
 
 
 class Transmit(ctypes.Structure):
@@ -94,6 +94,8 @@ def load(build_if_missing: bool = True):
     lib.das_execute.argtypes = [vp, vp, vp, vp]
     lib.das_beamform_host.restype = ctypes.c_int
     lib.das_beamform_host.argtypes = [vp, vp, vp, vp]
+    lib.das_plan_count_work.restype = ctypes.c_int
+    lib.das_plan_count_work.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong), ctypes.POINTER(ctypes.c_ulonglong)]
     lib.das_status_string.restype = ctypes.c_char_p
     lib.das_status_string.argtypes = [ctypes.c_int]
     lib.das_last_error.restype = ctypes.c_char_p
@@ -200,6 +202,12 @@ class Plan:
     def beamform_host(self, h_raw: int, h_out: int, stream: int = 0):
         _check(self._lib.das_beamform_host(self._h, ctypes.c_void_p(h_raw), ctypes.c_void_p(h_out),
                                            ctypes.c_void_p(stream)))
+
+    def count_work(self):
+        """(n_pairs, n_terms) of das_plan_count_work: active (m, n) pairs and entered (q, m, n) terms."""
+        a, b = ctypes.c_ulonglong(), ctypes.c_ulonglong()
+        _check(self._lib.das_plan_count_work(self._h, ctypes.byref(a), ctypes.byref(b)))
+        return int(a.value), int(b.value)
 
     def destroy(self):
         if getattr(self, "_h", None) is not None and self._h.value:

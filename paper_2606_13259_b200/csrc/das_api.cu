@@ -291,5 +291,22 @@ das_status_t das_beamform_host(das_plan_t* p, const void* h_raw, void* h_out, vo
   return DAS_OK;
 }
 
+das_status_t das_plan_count_work(const das_plan_t* p, unsigned long long* n_pairs, unsigned long long* n_terms) {
+  if (!p || !n_pairs || !n_terms) { set_err("das_plan_count_work: NULL argument"); return DAS_ERR_INVALID_ARG; }
+  DeviceGuard g(p->device);
+  if (!g.ok) return cuda_fail(g.err, "selecting the CUDA device");
+  unsigned long long* d = nullptr;
+  cudaError_t e = cudaMalloc(&d, 2 * sizeof(unsigned long long));
+  if (e != cudaSuccess) { cuda_fail(e, "allocating counters"); return DAS_ERR_ALLOC; }
+  unsigned long long h[2] = {0, 0};
+  if ((e = cudaMemset(d, 0, sizeof(h))) == cudaSuccess && (e = launch_count(p->P, d, nullptr)) == cudaSuccess)
+    e = cudaMemcpy(h, d, sizeof(h), cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (e != cudaSuccess) return cuda_fail(e, "das_plan_count_work");
+  *n_pairs = h[0];
+  *n_terms = h[1];
+  return DAS_OK;
+}
+
 #pragma GCC visibility pop
 }  // extern "C"

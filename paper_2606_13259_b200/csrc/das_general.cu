@@ -130,7 +130,76 @@ general_kernel(const Params P, const T* __restrict__ conv, void* __restrict__ ou
   else    reinterpret_cast<float*>(out_v)[n] = tot_re;
 }
 
+// Work counter (accounting for the bench's roofline, not part of the hot path): the number of
+// (m, n) pairs with non-zero receive weight and the number of (q, m, n) terms that enter the sum
+// (non-zero weight and 0 <= k <= K-2), classified by exactly the FP64 expressions of the general
+// kernel above.  One thread per voxel, warp-shuffle + one atomicAdd per warp.
+__global__ void __launch_bounds__(kThreads)
+count_kernel(const Params P, unsigned long long* __restrict__ counters) {
+  const long long N = (long long)P.nx * P.ny * P.nz;
+  const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  unsigned long long pairs = 0, terms = 0;
+  if (n < N) {
+    const int iz = (int)(n % P.nz);
+    const int iy = (int)((n / P.nz) % P.ny);
+    const int ix = (int)(n / ((long long)P.nz * P.ny));
+    const double px = (double)P.xs[ix], py = (double)P.ys[iy], pz = (double)P.zs[iz];
+    const double inv_c = 1.0 / P.c;
+    const double lim_hi = (double)(P.K - 2);
+    const double four_f2 = __dmul_rn(__dmul_rn(4.0, P.fnum), P.fnum);
+    for (int m = 0; m < P.M; ++m) {
+      const float4 e = __ldg(&P.elem[m]);
+      const double dx = px - (double)e.x, dy = py - (double)e.y, dz = pz - (double)e.z;
+      const double dx2 = __dmul_rn(dx, dx), dy2 = __dmul_rn(dy, dy), dz2 = __dmul_rn(dz, dz);
+      const double dd = __dadd_rn(__dadd_rn(dx2, dy2), dz2);
+      if (P.apod) {
+        double a, rho2;
+        if (P.has_dir) {
+          const float4 d = __ldg(&P.edir[m]);
+          a = __dadd_rn(__dadd_rn(__dmul_rn(dx, (double)d.x), __dmul_rn(dy, (double)d.y)),
+                        __dmul_rn(dz, (double)d.z));
+          rho2 = __dadd_rn(dd, -__dmul_rn(a, a));
+        } else {
+          a = dz;
+          rho2 = __dadd_rn(dx2, dy2);
+        }
+        if (!(a > 0.0 && __dmul_rn(four_f2, rho2) <= __dmul_rn(a, a))) continue;
+      }
+      ++pairs;
+      const double tau_rx = sqrt(dd) * inv_c;
+      for (int q = 0; q < P.Q; ++q) {
+        const TxDev tx = P.tx[q];
+        double tau_tx;
+        if (tx.type == DAS_TX_PLANE) {
+          tau_tx = (px * tx.vx + py * tx.vy + pz * tx.vz) * inv_c + tx.t0;
+        } else {
+          const double ax = px - tx.vx, ay = py - tx.vy, az = pz - tx.vz;
+          tau_tx = sqrt(ax * ax + ay * ay + az * az) * inv_c + tx.t0;
+        }
+        const double kf = floor((tau_tx + tau_rx - P.t_start) * P.fs);
+        if (kf >= 0.0 && kf <= lim_hi) ++terms;
+      }
+    }
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    pairs += __shfl_down_sync(0xffffffffu, pairs, o);
+    terms += __shfl_down_sync(0xffffffffu, terms, o);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    atomicAdd(&counters[0], pairs);
+    atomicAdd(&counters[1], terms);
+  }
+}
+
 }  // namespace
+
+cudaError_t launch_count(const Params& P, unsigned long long* d_counters, cudaStream_t s) {
+  const long long N = (long long)P.nx * P.ny * P.nz;
+  const unsigned blocks = (unsigned)((N + kThreads - 1) / kThreads);
+  count_kernel<<<blocks, kThreads, 0, s>>>(P, d_counters);
+  count_launch();
+  return cudaGetLastError();
+}
 
 cudaError_t launch_general(const Params& P, const void* d_conv, void* d_out, cudaStream_t s) {
   const long long N = (long long)P.nx * P.ny * P.nz;

@@ -59,6 +59,7 @@ struct Params {
 cudaError_t launch_convert(const Params& P, const void* d_raw, void* d_conv, float scale,
                            cudaStream_t s);
 cudaError_t launch_general(const Params& P, const void* d_conv, void* d_out, cudaStream_t s);
+cudaError_t launch_count(const Params& P, unsigned long long* d_counters, cudaStream_t s);
 
 struct TiledPlan;      // opaque to the API layer (das_tiled.cu)
 // Returns nullptr and fills why[] if the geometry does not qualify for the tiled kernel.

@@ -75,6 +75,7 @@ def test_null_arguments(das_lib):
     assert lib.das_convert(None, None, None, 1.0, None) == das_lib.ERR_INVALID_ARG
     assert lib.das_execute(None, None, None, None) == das_lib.ERR_INVALID_ARG
     assert lib.das_beamform_host(None, None, None, None) == das_lib.ERR_INVALID_ARG
+    assert lib.das_plan_count_work(None, None, None) == das_lib.ERR_INVALID_ARG
     assert lib.das_converted_bytes(None) == 0
     assert das_lib.status_string(0) == "DAS_OK"
 

@@ -343,3 +343,33 @@ def test_execute_overwrites_output_and_is_repeatable(das_lib):
     plan.execute(conv.data_ptr(), out.data_ptr())
     assert das.launch_count() > n0
     plan.destroy()
+
+
+# ------------------------------------------------------------------ work counter (integers: bit-exact)
+
+@pytest.mark.parametrize("number", [1, 2])
+def test_count_work_matches_oracle(das_lib, number):
+    """das_plan_count_work (the bench's accounting) against the oracle's per-voxel term count
+    (pin P5): integer work, so the totals must be identical.  Every sample of
+    configs 1 and 2 is in range, so entered terms = Q x active pairs."""
+    import oracle
+    w = _cfg(number)
+    cnt = oracle.das(w, want_count=True)["count"]
+    plan = das_lib.Plan.from_workload(w)
+    pairs, terms = plan.count_work()
+    plan.destroy()
+    assert terms == int(cnt.sum())
+    assert pairs * w.n_tx == terms
+
+
+def test_count_work_out_of_range(das_lib):
+    import oracle
+    base = _subgrid(2, slice(28, 34), slice(30, 35), slice(8, 56))
+    w = wl.custom(base.elem_pos, base.tx_type, base.tx_v, base.tx_t0, base.xs, base.ys, base.zs,
+                  fs=base.fs, n_samples=120, t_start=5.0e-6, f_number=1.0,
+                  y=np.ascontiguousarray(base.y[:, :, 40:160]))
+    cnt = oracle.das(w, want_count=True)["count"]
+    plan = das_lib.Plan.from_workload(w)
+    pairs, terms = plan.count_work()
+    plan.destroy()
+    assert terms == int(cnt.sum()) and terms < pairs * w.n_tx
