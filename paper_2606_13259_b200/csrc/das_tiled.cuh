@@ -14,43 +14,53 @@
 // an f/1 cone), so FP32 keeps ~1e-6 samples on it.
 //
 // Work split inside a CTA (one CTA = one voxel tile at a time, persistent over a static,
-// work-sorted tile list):
+// work-sorted tile list); three warp roles connected by two mbarrier rings:
 //   * ONE producer warp walks the tile's active-receiver list (built by the plan).  For each
-//     receiver m it issues, per transmit q of the current chunk, one TMA bulk copy
-//     (cp.async.bulk global -> shared, completion counted on an mbarrier) of the W table entries
-//     [k0, k0 + W), k0 = K0tile_q + E0_m, of row (m, q) of the converted channel data.  The
-//     entries are already (mid, slope) pairs with zeros outside the valid sample range
-//     (das_internal.cuh), so staging is a pure copy: no producer arithmetic, no bounds tests.
+//     receiver m it issues, per transmit q, one TMA bulk copy (cp.async.bulk global -> shared,
+//     completion counted on an mbarrier) of the W table entries [k0, k0 + W),
+//     k0 = K0tile_q + E0_m, of row (m, q) of the converted channel data (storage precision,
+//     (mid, slope) pairs, zeros outside the valid sample range: das_internal.cuh) into the RAW
+//     ring.
+//   * CONVERTER warps turn one raw stage into one stage of the TABLE ring: FP32 line
+//     coefficients in window-local coordinates, entry i = (c_i, slope_i) with
+//     c_i = mid_i - i * slope_i, so that the interpolated sample at local position ts
+//     (already shifted by -1/2) is  y = c_i + ts * slope_i : ONE fused multiply-add per
+//     component with the position itself as the multiplier (no fraction to extract), FP32
+//     whatever the storage precision ("converted to FP32 before interpolation").
+//     This costs 4 conversions per staged entry instead of 2 per accumulated term.
 //   * consumer threads own one voxel each (a warp = 8 x 4 lateral voxels at one depth, so all
 //     lanes read nearly the same shared-memory words: broadcast), keep QC complex accumulators
 //     and QC reduced transmit delays in registers, and run the (m outer, q inner) loop:
-//       ts = Tf_q + e'          u = ts + MAGIC (rounds to the entry index)   al = ts - (u - MAGIC)
-//       (mid, slope) = table[u]             s = mid + al * slope            acc_q += Prx * s
-//     Index arithmetic and the complex multiply-accumulate are issued as packed FP32x2
-//     instructions (FADD2 / FFMA2, new on sm_100) over pairs of transmits.
-//   * stages travel through an mbarrier ring (full: expect_tx + TMA complete_tx; empty: one
-//     arrive per consumer warp), so L2 latency is hidden behind the consumers' arithmetic.
+//       ts = Tf_q + e'     u = ts + MAGIC (its low mantissa bits are the rounded entry index)
+//       (c, slope) = table[bits(u)]     s = c + ts * slope     acc_q += Prx * s
+// Helper warps give most of their registers to the consumers (setmaxnreg).
 #pragma once
 
 #include "das_internal.cuh"
 
 namespace das {
 
-constexpr int kStages = 8;
+constexpr int kRawStages = 4;                   // ring of TMA-staged windows (storage precision)
+constexpr int kTabStages = 4;                   // ring of FP32 line tables the consumers read
+constexpr int kConvWarps = 2;
+constexpr int kHelperWarps = 4;                 // one warpgroup: producer + converters (+ idle)
 constexpr int kLaneX = 8, kLaneY = 4;          // a consumer warp covers 8 x 4 lateral voxels
 constexpr int kWX = 1, kWY = 2, kWZ = 4;       // consumer warps per tile: tile = 8 x 8 x 4 voxels
 constexpr int kConsumerWarps = kWX * kWY * kWZ;
-constexpr int kTiledThreads = (kConsumerWarps + 1) * 32;
+constexpr int kConsumerThreads = kConsumerWarps * 32;
+constexpr int kTiledThreads = (kConsumerWarps + kHelperWarps) * 32;
+constexpr int kRegsConsumer = 96, kRegsHelper = 40;    // 256 * 96 + 128 * 40 <= 384 * 80
 constexpr float kMagic = 12582912.0f;           // 1.5 * 2^23: adding it rounds to an integer
 constexpr unsigned kMagicBits = 0x4B400000u;
 constexpr float kBand = 4e-6f;                  // relative guard band of the FP32 aperture test
+static_assert(kConsumerWarps % 4 == 0 && kHelperWarps == 4 && kConvWarps + 1 <= kHelperWarps, "warpgroup roles");
 
 enum Mode { kIQ32 = 0, kIQ16 = 1, kRF32 = 2, kRF16 = 3 };
-template <int MODE> struct ModeTraits;
-template <> struct ModeTraits<kIQ32> { static constexpr bool iq = true;  static constexpr int eb = 16; };
-template <> struct ModeTraits<kIQ16> { static constexpr bool iq = true;  static constexpr int eb = 8; };
-template <> struct ModeTraits<kRF32> { static constexpr bool iq = false; static constexpr int eb = 8; };
-template <> struct ModeTraits<kRF16> { static constexpr bool iq = false; static constexpr int eb = 4; };
+template <int MODE> struct ModeTraits;   // eb: bytes of a stored (mid, slope) entry; tb: of a table entry
+template <> struct ModeTraits<kIQ32> { static constexpr bool iq = true;  static constexpr int eb = 16, tb = 16; };
+template <> struct ModeTraits<kIQ16> { static constexpr bool iq = true;  static constexpr int eb = 8,  tb = 16; };
+template <> struct ModeTraits<kRF32> { static constexpr bool iq = false; static constexpr int eb = 8,  tb = 8; };
+template <> struct ModeTraits<kRF16> { static constexpr bool iq = false; static constexpr int eb = 4,  tb = 8; };
 __host__ __device__ inline int entry_bytes(int iq, int fp16) { return (iq ? 2 : 1) * 2 * (fp16 ? 2 : 4); }
 
 struct TileDesc {       // one voxel tile
@@ -104,16 +114,29 @@ template <int OFF> __device__ __forceinline__ float4 lds128(unsigned addr) {
   asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4+%5];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr), "n"(OFF));
   return v;
 }
-template <int OFF> __device__ __forceinline__ uint2 lds64(unsigned addr) {
+template <int OFF> __device__ __forceinline__ float2 lds64f(unsigned addr) {
+  float2 v;
+  asm volatile("ld.shared.v2.f32 {%0,%1}, [%2+%3];" : "=f"(v.x), "=f"(v.y) : "r"(addr), "n"(OFF));
+  return v;
+}
+__device__ __forceinline__ uint2 lds64u(unsigned addr) {
   uint2 v;
-  asm volatile("ld.shared.v2.b32 {%0,%1}, [%2+%3];" : "=r"(v.x), "=r"(v.y) : "r"(addr), "n"(OFF));
+  asm volatile("ld.shared.v2.b32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
   return v;
 }
-template <int OFF> __device__ __forceinline__ unsigned lds32(unsigned addr) {
+__device__ __forceinline__ unsigned lds32u(unsigned addr) {
   unsigned v;
-  asm volatile("ld.shared.b32 %0, [%1+%2];" : "=r"(v) : "r"(addr), "n"(OFF));
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v) : "r"(addr));
   return v;
 }
+__device__ __forceinline__ void sts128(unsigned addr, float4 v) {
+  asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ void sts64(unsigned addr, float2 v) {
+  asm volatile("st.shared.v2.f32 [%0], {%1,%2};" ::"r"(addr), "f"(v.x), "f"(v.y) : "memory");
+}
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 __device__ __forceinline__ float rsqrt_approx(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float rcp_approx(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float sin_approx(float x) { float r; asm("sin.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
@@ -121,11 +144,20 @@ __device__ __forceinline__ float cos_approx(float x) { float r; asm("cos.approx.
 
 template <int QC, int W, int MODE>
 struct alignas(128) TiledSmem {
-  unsigned char tab[kStages][QC * W * ModeTraits<MODE>::eb];
-  float4 meta[kStages];                 // (ex, ey, E0, unused) of the staged receiver
-  unsigned long long full[kStages];
-  unsigned long long empty[kStages];
+  unsigned char tab[kTabStages][QC * W * ModeTraits<MODE>::tb];
+  unsigned char raw[kRawStages][QC * W * ModeTraits<MODE>::eb];
+  float cyc[ModeTraits<MODE>::iq ? QC : 1][kConsumerThreads];   // transmit phase (cycles) per (q, voxel)
+  float4 meta_raw[kRawStages];          // (ex, ey, E0, -) of the staged receiver
+  float4 meta_tab[kTabStages];          // (ex, ey, E0, MAGIC + first entry of the stage)
+  unsigned long long raw_full[kRawStages], raw_empty[kRawStages];
+  unsigned long long tab_full[kTabStages], tab_empty[kTabStages];
 };
+
+// upper bound of sizeof(TiledSmem<QC, W, MODE>) for the plan's occupancy estimate
+__host__ __device__ inline size_t tiled_smem_bytes(int QC, int W, int iq, int fp16) {
+  const size_t tb = iq ? 16 : 8, eb = (size_t)entry_bytes(iq, fp16);
+  return (size_t)QC * W * (kTabStages * tb + kRawStages * eb) + (size_t)(iq ? QC : 1) * kConsumerThreads * 4 + 512;
+}
 
 // exact (definition-order, FP64) aperture test for pairs inside the FP32 guard band
 static __device__ __noinline__ bool aperture_exact(float x, float y, float ex, float ey, double a, double fnum) {
@@ -141,35 +173,22 @@ __device__ __forceinline__ double tx_delay(const TxDev& tx, double x, double y, 
   return sqrt(bx * bx + by * by + bz * bz) / c + tx.t0;
 }
 
-// One interpolated sample per transmit of the pair (j, j+1): returns s (re, im) for each.
-template <int MODE, int OFF0, int OFF1>
-__device__ __forceinline__ void gather_pair(unsigned a0, unsigned a1, float2 al, float2& sre, float2& sim) {
-  if constexpr (MODE == kIQ32) {
-    const float4 v0 = lds128<OFF0>(a0);
-    const float4 v1 = lds128<OFF1>(a1);
-    sre = make_float2(fmaf(al.x, v0.z, v0.x), fmaf(al.y, v1.z, v1.x));
-    sim = make_float2(fmaf(al.x, v0.w, v0.y), fmaf(al.y, v1.w, v1.y));
-  } else if constexpr (MODE == kIQ16) {
-    const uint2 v0 = lds64<OFF0>(a0);
-    const uint2 v1 = lds64<OFF1>(a1);
-    const __half2 alh = __floats2half2_rn(al.x, al.y);
-    const __half2 s0 = __hfma2(__low2half2(alh), *reinterpret_cast<const __half2*>(&v0.y), *reinterpret_cast<const __half2*>(&v0.x));
-    const __half2 s1 = __hfma2(__high2half2(alh), *reinterpret_cast<const __half2*>(&v1.y), *reinterpret_cast<const __half2*>(&v1.x));
-    sre = make_float2(__low2float(s0), __low2float(s1));
-    sim = make_float2(__high2float(s0), __high2float(s1));
-  } else if constexpr (MODE == kRF32) {
-    const uint2 v0 = lds64<OFF0>(a0);
-    const uint2 v1 = lds64<OFF1>(a1);
-    sre = make_float2(fmaf(al.x, __uint_as_float(v0.y), __uint_as_float(v0.x)),
-                      fmaf(al.y, __uint_as_float(v1.y), __uint_as_float(v1.x)));
-    sim = make_float2(0.f, 0.f);
+// One accumulated term: gather the line of transmit row ROW at entry address a, interpolate at
+// ts, rotate by (pr, pi) and add.
+template <int MODE, int OFF>
+__device__ __forceinline__ void term(unsigned a, float ts, float pr, float pi, float& accR, float& accI) {
+  if constexpr (ModeTraits<MODE>::iq) {
+    const float4 v = lds128<OFF>(a);                 // (c.re, c.im, slope.re, slope.im)
+    const float sre = fmaf(ts, v.z, v.x);
+    const float sim = fmaf(ts, v.w, v.y);
+    accR = fmaf(sre, pr, accR);
+    accR = fmaf(-sim, pi, accR);
+    accI = fmaf(sre, pi, accI);
+    accI = fmaf(sim, pr, accI);
   } else {
-    const unsigned w0 = lds32<OFF0>(a0);
-    const unsigned w1 = lds32<OFF1>(a1);
-    const float2 f0 = __half22float2(*reinterpret_cast<const __half2*>(&w0));
-    const float2 f1 = __half22float2(*reinterpret_cast<const __half2*>(&w1));
-    sre = make_float2(fmaf(al.x, f0.y, f0.x), fmaf(al.y, f1.y, f1.x));
-    sim = make_float2(0.f, 0.f);
+    const float2 v = lds64f<OFF>(a);                 // (c, slope)
+    accR += v.x;
+    accR = fmaf(ts, v.y, accR);
   }
 }
 
@@ -177,66 +196,118 @@ template <int QC, int W, int MODE>
 __global__ void __launch_bounds__(kTiledThreads, 2)
 tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict__ conv, void* __restrict__ out_v) {
   constexpr bool IQ = ModeTraits<MODE>::iq;
-  constexpr int EB = ModeTraits<MODE>::eb;
-  constexpr int ESH = (EB == 16) ? 4 : (EB == 8) ? 3 : 2;
+  constexpr int EB = ModeTraits<MODE>::eb, TB = ModeTraits<MODE>::tb;
+  constexpr int TSH = (TB == 16) ? 4 : 3;
+  constexpr int NE = QC * W;                         // entries per stage
   constexpr int QP = (QC + 1) / 2;                   // transmit pairs per chunk
   extern __shared__ __align__(128) unsigned char smem_raw[];
   TiledSmem<QC, W, MODE>& sm = *reinterpret_cast<TiledSmem<QC, W, MODE>*>(smem_raw);
 
   const int tid = threadIdx.x;
   const int warp = tid >> 5, lane = tid & 31;
-  const unsigned full0 = smem_u32(&sm.full[0]), empty0 = smem_u32(&sm.empty[0]);
+  const unsigned raw_full0 = smem_u32(&sm.raw_full[0]), raw_empty0 = smem_u32(&sm.raw_empty[0]);
+  const unsigned tab_full0 = smem_u32(&sm.tab_full[0]), tab_empty0 = smem_u32(&sm.tab_empty[0]);
   if (tid == 0) {
-    for (int s = 0; s < kStages; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, kConsumerWarps); }
+    for (int s = 0; s < kRawStages; ++s) { mbar_init(raw_full0 + 8 * s, 1); mbar_init(raw_empty0 + 8 * s, 1); }
+    for (int s = 0; s < kTabStages; ++s) { mbar_init(tab_full0 + 8 * s, 1); mbar_init(tab_empty0 + 8 * s, kConsumerWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
 
-  unsigned seq = 0;          // stages produced / consumed so far by this CTA (same count on both sides)
+  unsigned seq = 0;          // receiver stages produced / converted / consumed so far by this CTA
 
-  if (warp == kConsumerWarps) {
-    // =============================== PRODUCER (TMA) =========================================
-    const unsigned tab0 = smem_u32(&sm.tab[0][0]);
-    for (int tile_i = blockIdx.x; tile_i < tp.n_tiles; tile_i += gridDim.x) {
-      const TileDesc td = tp.tiles[tile_i];
-      for (int ch = 0; ch < tp.n_chunks; ++ch) {
-        const int q = ch * QC + lane;
-        const bool qok = lane < QC && q < P.Q;
-        const int k0 = qok ? __ldg(&tp.k0tile[(long long)tile_i * P.Q + q]) : 0;
-        const int nq = min(QC, P.Q - ch * QC);
-        for (int li = 0; li < td.list_cnt; ++li, ++seq) {
-          const unsigned slot = seq % kStages;
-          const unsigned ent = __ldg(&tp.list[td.list_off + li]);
-          const int m = (int)(ent & 0xFFFFu);
-          const int e0 = (int)(ent >> 16);
-          const float4 el = __ldg(&P.elem[m]);
-          mbar_wait(empty0 + 8 * slot, ((seq / kStages) & 1u) ^ 1u);
-          if (lane == 0) {
-            sm.meta[slot] = make_float4(el.x, el.y, (float)e0, 0.f);
-            mbar_arrive_expect_tx(full0 + 8 * slot, (unsigned)(nq * W * EB));
-          }
-          __syncwarp();
-          if (qok) {
-            int i0 = kPadLeft + k0 + e0;                  // first table entry of the window
-            i0 = max(0, min(i0, P.Kp - W));               // clamped windows lie entirely in a zero pad
-            const unsigned char* src = conv + (((long long)m * P.Q + q) * P.Kp + i0) * EB;
-            tma_bulk_g2s(tab0 + slot * (QC * W * EB) + lane * (W * EB), src, W * EB, full0 + 8 * slot);
+  if (warp >= kConsumerWarps) {
+    reg_dec<kRegsHelper>();
+    const int hw = warp - kConsumerWarps;
+    if (hw == 0) {
+      // =============================== PRODUCER (TMA) =======================================
+      const unsigned raw0 = smem_u32(&sm.raw[0][0]);
+      for (int tile_i = blockIdx.x; tile_i < tp.n_tiles; tile_i += gridDim.x) {
+        const TileDesc td = tp.tiles[tile_i];
+        for (int ch = 0; ch < tp.n_chunks; ++ch) {
+          const int q = ch * QC + lane;
+          const bool qok = lane < QC && q < P.Q;
+          const int k0 = qok ? __ldg(&tp.k0tile[(long long)tile_i * P.Q + q]) : 0;
+          const int nq = min(QC, P.Q - ch * QC);
+          for (int li = 0; li < td.list_cnt; ++li, ++seq) {
+            const unsigned slot = seq % kRawStages;
+            const unsigned ent = __ldg(&tp.list[td.list_off + li]);
+            const int m = (int)(ent & 0xFFFFu);
+            const int e0 = (int)(ent >> 16);
+            const float4 el = __ldg(&P.elem[m]);
+            mbar_wait(raw_empty0 + 8 * slot, ((seq / kRawStages) & 1u) ^ 1u);
+            if (lane == 0) {
+              sm.meta_raw[slot] = make_float4(el.x, el.y, (float)e0, 0.f);
+              mbar_arrive_expect_tx(raw_full0 + 8 * slot, (unsigned)(nq * W * EB));
+            }
+            __syncwarp();
+            if (qok) {
+              int i0 = kPadLeft + k0 + e0;                  // first table entry of the window
+              i0 = max(0, min(i0, P.Kp - W));               // clamped windows lie entirely in a zero pad
+              const unsigned char* src = conv + (((long long)m * P.Q + q) * P.Kp + i0) * EB;
+              tma_bulk_g2s(raw0 + slot * (NE * EB) + lane * (W * EB), src, W * EB, raw_full0 + 8 * slot);
+            }
           }
         }
+      }
+    } else if (hw <= kConvWarps) {
+      // =============================== CONVERTERS ===========================================
+      const unsigned cw = (unsigned)(hw - 1);
+      const unsigned raw0 = smem_u32(&sm.raw[0][0]), tab0 = smem_u32(&sm.tab[0][0]);
+      for (int tile_i = blockIdx.x; tile_i < tp.n_tiles; tile_i += gridDim.x) {
+        const unsigned end = seq + (unsigned)(tp.tiles[tile_i].list_cnt * tp.n_chunks);
+        for (unsigned s = seq + (cw + kConvWarps - seq % kConvWarps) % kConvWarps; s < end; s += kConvWarps) {
+          const unsigned rs = s % kRawStages, ts = s % kTabStages;
+          mbar_wait(raw_full0 + 8 * rs, (s / kRawStages) & 1u);
+          mbar_wait(tab_empty0 + 8 * ts, ((s / kTabStages) & 1u) ^ 1u);
+          if (lane == 0) {
+            float4 mt = sm.meta_raw[rs];
+            mt.w = kMagic + (float)(ts * NE);
+            sm.meta_tab[ts] = mt;
+          }
+          const unsigned src = raw0 + rs * (NE * EB) + lane * EB, dst = tab0 + ts * (NE * TB) + lane * TB;
+#pragma unroll
+          for (int j = 0; j < (NE + 31) / 32; ++j) {
+            const int e = lane + 32 * j;
+            if (NE % 32 == 0 || e < NE) {
+              const float kl = (float)(e % W);               // window-local entry index
+              if constexpr (MODE == kIQ16) {
+                const uint2 r = lds64u(src + j * 32 * EB);
+                const float2 mid = __half22float2(*reinterpret_cast<const __half2*>(&r.x));
+                const float2 sl = __half22float2(*reinterpret_cast<const __half2*>(&r.y));
+                sts128(dst + j * 32 * TB, make_float4(fmaf(-kl, sl.x, mid.x), fmaf(-kl, sl.y, mid.y), sl.x, sl.y));
+              } else if constexpr (MODE == kIQ32) {
+                const float4 r = lds128<0>(src + j * 32 * EB);
+                sts128(dst + j * 32 * TB, make_float4(fmaf(-kl, r.z, r.x), fmaf(-kl, r.w, r.y), r.z, r.w));
+              } else if constexpr (MODE == kRF16) {
+                const unsigned r = lds32u(src + j * 32 * EB);
+                const float2 ms = __half22float2(*reinterpret_cast<const __half2*>(&r));
+                sts64(dst + j * 32 * TB, make_float2(fmaf(-kl, ms.y, ms.x), ms.y));
+              } else {
+                const float2 r = lds64f<0>(src + j * 32 * EB);
+                sts64(dst + j * 32 * TB, make_float2(fmaf(-kl, r.y, r.x), r.y));
+              }
+            }
+          }
+          __syncwarp();
+          if (lane == 0) { mbar_arrive(tab_full0 + 8 * ts); mbar_arrive(raw_empty0 + 8 * rs); }
+        }
+        seq = end;
       }
     }
     return;
   }
 
   // ================================= CONSUMERS ==============================================
+  reg_inc<kRegsConsumer>();
   const int wz = warp / (kWX * kWY), wy = (warp / kWX) % kWY, wx = warp % kWX;
   const int lx = lane % kLaneX, ly = lane / kLaneX;
   const float kappa = (float)tp.kappa;
   const float ratio = (float)tp.ratio;
-  // table address of entry index bits: (bits(u) << ESH) + base_adj, where bits(u) still holds
+  // table address of entry index bits: (bits(u) << TSH) + base_adj, where bits(u) still holds
   // the float exponent pattern of MAGIC; base_adj removes it (mod 2^32)
-  unsigned base_adj = smem_u32(&sm.tab[0][0]) - (kMagicBits << ESH);
-  asm volatile("mov.b32 %0, %0;" : "+r"(base_adj));     // opaque: keeps (bits << ESH) + base one LEA
+  unsigned base_adj = smem_u32(&sm.tab[0][0]) - (kMagicBits << TSH);
+  asm volatile("mov.b32 %0, %0;" : "+r"(base_adj));     // opaque: keeps (bits << TSH) + base one LEA
 
   for (int tile_i = blockIdx.x; tile_i < tp.n_tiles; tile_i += gridDim.x) {
     const TileDesc td = tp.tiles[tile_i];
@@ -252,29 +323,30 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
 
     for (int ch = 0; ch < tp.n_chunks; ++ch) {
       const int q0 = ch * QC;
-      // ---- per-(q, n) part in FP64: reduced transmit delay -------------------------------
+      // ---- per-(q, n) part in FP64: reduced transmit delay and transmit phase -------------
       float2 Tf[QP];
-      float2 accR[QP], accI[QP];          // (acc_j, acc_j+1) real and imaginary parts
+      float accR[2 * QP], accI[2 * QP];
 #pragma unroll
-      for (int jp = 0; jp < QP; ++jp) {
-        float tf[2];
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          const int q = min(q0 + 2 * jp + h, P.Q - 1);
-          const double T = (tx_delay(P.tx[q], x, y, z, P.c) + a_d / P.c - P.t_start) * P.fs;
-          const int k0 = __ldg(&tp.k0tile[(long long)tile_i * P.Q + q]);
-          tf[h] = (float)(T - (double)k0 - 0.5);
+      for (int j = 0; j < 2 * QP; ++j) {
+        const int q = min(q0 + j, P.Q - 1);
+        const double T = (tx_delay(P.tx[q], x, y, z, P.c) + a_d / P.c - P.t_start) * P.fs;
+        const int k0 = __ldg(&tp.k0tile[(long long)tile_i * P.Q + q]);
+        const float tf = (float)(T - (double)k0 - 0.5);
+        if (j & 1) Tf[j >> 1].y = tf; else Tf[j >> 1].x = tf;
+        if (IQ && j < QC) {
+          double cyc = tp.phase0 + tp.ratio * T;
+          cyc -= rint(cyc);
+          sm.cyc[IQ ? j : 0][tid] = (float)cyc;          // read back by this thread only
         }
-        Tf[jp] = make_float2(tf[0], tf[1]);
-        accR[jp] = make_float2(0.f, 0.f);
-        accI[jp] = make_float2(0.f, 0.f);
+        accR[j] = 0.f;
+        accI[j] = 0.f;
       }
 
       // ---- receiver loop ---------------------------------------------------------------
       for (int li = 0; li < td.list_cnt; ++li, ++seq) {
-        const unsigned slot = seq % kStages;
-        mbar_wait(full0 + 8 * slot, (seq / kStages) & 1u);
-        const float4 meta = sm.meta[slot];
+        const unsigned slot = seq % kTabStages;
+        mbar_wait(tab_full0 + 8 * slot, (seq / kTabStages) & 1u);
+        const float4 meta = sm.meta_tab[slot];
         const float dx = x - meta.x, dy = y - meta.y;
         const float rho2 = fmaf(dx, dx, dy * dy);
         bool act = in_grid;
@@ -297,61 +369,40 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
             pr = cos_approx(ang);
             pi = sin_approx(ang);
           }
-          const float magic = kMagic + (float)(slot * (QC * W));
-          const float2 ep2 = make_float2(ep, ep), mg2 = make_float2(magic, magic), nmg2 = make_float2(-magic, -magic);
-          const float2 neg1 = make_float2(-1.f, -1.f);
-          const float2 prr = make_float2(pr, pr), pii = make_float2(pi, pi), npi = make_float2(-pi, -pi);
+          const float2 ep2 = make_float2(ep, ep), mg2 = make_float2(meta.w, meta.w);
+          constexpr int kRow = W * TB;
 #pragma unroll
           for (int jp = 0; jp < QP; ++jp) {
             const float2 ts = __fadd2_rn(Tf[jp], ep2);
             const float2 u = __fadd2_rn(ts, mg2);
-            const float2 kf = __fadd2_rn(u, nmg2);
-            const float2 al = __ffma2_rn(kf, neg1, ts);
-            const unsigned a0 = (__float_as_uint(u.x) << ESH) + base_adj;
-            const unsigned a1 = (__float_as_uint(u.y) << ESH) + base_adj;
-            float2 sre, sim;
-            constexpr int kRow = W * EB;
+            const unsigned a0 = (__float_as_uint(u.x) << TSH) + base_adj;
+            const unsigned a1 = (__float_as_uint(u.y) << TSH) + base_adj;
             // immediates: row offsets of transmit 2 jp and 2 jp + 1 inside a stage
             switch (jp) {
-#define DAS_CASE(JP) case JP: gather_pair<MODE, (2 * JP) * kRow, ((2 * JP + 1) % (QC > 1 ? QC : 1)) * kRow>(a0, a1, al, sre, sim); break;
+#define DAS_CASE(JP) case JP: \
+              term<MODE, (2 * JP) * kRow>(a0, ts.x, pr, pi, accR[2 * jp], accI[2 * jp]); \
+              term<MODE, ((2 * JP + 1) % (QC > 1 ? QC : 1)) * kRow>(a1, ts.y, pr, pi, accR[2 * jp + 1], accI[2 * jp + 1]); break;
               DAS_CASE(0) DAS_CASE(1) DAS_CASE(2) DAS_CASE(3) DAS_CASE(4) DAS_CASE(5) DAS_CASE(6) DAS_CASE(7)
 #undef DAS_CASE
-              default: sre = sim = make_float2(0.f, 0.f);
-            }
-            if (IQ) {
-              accR[jp] = __ffma2_rn(sre, prr, accR[jp]);
-              accR[jp] = __ffma2_rn(sim, npi, accR[jp]);
-              accI[jp] = __ffma2_rn(sre, pii, accI[jp]);
-              accI[jp] = __ffma2_rn(sim, prr, accI[jp]);
-            } else {
-              accR[jp] = __fadd2_rn(accR[jp], sre);
+              default: break;
             }
           }
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(empty0 + 8 * slot);
+        if (lane == 0) mbar_arrive(tab_empty0 + 8 * slot);
       }
 
       // ---- fold this chunk: x += sum_q Ptx_q * acc_q ---------------------------------------
 #pragma unroll
-      for (int jp = 0; jp < QP; ++jp) {
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          const int q = q0 + 2 * jp + h;
-          if (2 * jp + h < QC && q < P.Q) {
-            const float are = h ? accR[jp].y : accR[jp].x;
-            const float aim = h ? accI[jp].y : accI[jp].x;
-            if (IQ) {
-              const double T = (tx_delay(P.tx[q], x, y, z, P.c) + a_d / P.c - P.t_start) * P.fs;
-              double cyc = tp.phase0 + tp.ratio * T;
-              cyc -= rint(cyc);
-              float sn, cs;
-              sincospif(2.0f * (float)cyc, &sn, &cs);
-              out_re = fmaf(are, cs, fmaf(-aim, sn, out_re));
-              out_im = fmaf(are, sn, fmaf(aim, cs, out_im));
-            } else {
-              out_re += are;
-            }
+      for (int j = 0; j < 2 * QP; ++j) {
+        if (j < QC && q0 + j < P.Q) {
+          if (IQ) {
+            const float ang = 6.283185307179586f * sm.cyc[IQ ? j : 0][tid];
+            const float cs = cos_approx(ang), sn = sin_approx(ang);
+            out_re = fmaf(accR[j], cs, fmaf(-accI[j], sn, out_re));
+            out_im = fmaf(accR[j], sn, fmaf(accI[j], cs, out_im));
+          } else {
+            out_re += accR[j];
           }
         }
       }

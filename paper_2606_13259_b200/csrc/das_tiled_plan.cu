@@ -158,8 +158,8 @@ TiledPlan* tiled_plan_create(const Params& P, const das_plan_desc_t& d, int devi
   cudaDeviceProp prop;
   cudaError_t e = cudaGetDeviceProperties(&prop, device);
   if (e != cudaSuccess) { *cuda_err = e; delete tp; return nullptr; }
-  const size_t smem = (size_t)kStages * QC * W * entry_bytes(P.iq, P.fp16) + 1024;
-  const int ctas_per_sm = smem * 2 <= 200 * 1024 ? 2 : 1;
+  const size_t smem = tiled_smem_bytes(QC, W, P.iq, P.fp16);
+  const int ctas_per_sm = (smem + 1024) * 2 <= (size_t)prop.sharedMemPerMultiprocessor ? 2 : 1;
   tp->grid = std::max(1, std::min(n_tiles, prop.multiProcessorCount * ctas_per_sm));
   TiledDev& dv = tp->dev;
   dv.n_tiles = n_tiles;
