@@ -49,7 +49,7 @@ constexpr int kWX = 1, kWY = 2, kWZ = 4;       // consumer warps per tile: tile 
 constexpr int kConsumerWarps = kWX * kWY * kWZ;
 constexpr int kConsumerThreads = kConsumerWarps * 32;
 constexpr int kTiledThreads = (kConsumerWarps + kHelperWarps) * 32;
-constexpr int kRegsConsumer = 96, kRegsHelper = 40;    // 256 * 96 + 128 * 40 <= 384 * 80
+constexpr int kRegsConsumer = 104, kRegsHelper = 32;   // 256 * 104 + 128 * 32 <= 384 * 80
 constexpr float kMagic = 12582912.0f;           // 1.5 * 2^23: adding it rounds to an integer
 constexpr unsigned kMagicBits = 0x4B400000u;
 constexpr float kBand = 4e-6f;                  // relative guard band of the FP32 aperture test
@@ -80,6 +80,9 @@ struct TiledDev {
   double ratio;               // fc / fs
   double phase0;              // frac(fc * t_start), cycles
   float four_f2;              // 4 f#^2
+  float kappa_f, ratio_f;     // float copies (no F2F conversions in the receiver loop)
+  unsigned addr_bias;         // -(bits(MAGIC) << log2(table entry bytes)) mod 2^32: a kernel PARAMETER so
+                              // that ptxas cannot split (bits(u) << s) + base into LEA + IADD
 };
 
 // ---- PTX helpers ---------------------------------------------------------------------------
@@ -137,6 +140,7 @@ __device__ __forceinline__ void sts64(unsigned addr, float2 v) {
 }
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+__device__ __forceinline__ float pin(float v) { return __shfl_sync(0xffffffffu, v, threadIdx.x & 31); }
 __device__ __forceinline__ float rsqrt_approx(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float rcp_approx(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float sin_approx(float x) { float r; asm("sin.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
@@ -160,7 +164,8 @@ __host__ __device__ inline size_t tiled_smem_bytes(int QC, int W, int iq, int fp
 }
 
 // exact (definition-order, FP64) aperture test for pairs inside the FP32 guard band
-static __device__ __noinline__ bool aperture_exact(float x, float y, float ex, float ey, double a, double fnum) {
+static __device__ __noinline__ bool aperture_exact(float x, float y, float ex, float ey, const float* zs, int iz, double z_array, double fnum) {
+  const double a = (double)__ldg(&zs[iz]) - z_array;
   const double dx = (double)x - (double)ex, dy = (double)y - (double)ey;
   const double rho2 = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
   const double four_f2 = __dmul_rn(__dmul_rn(4.0, fnum), fnum);
@@ -173,22 +178,65 @@ __device__ __forceinline__ double tx_delay(const TxDev& tx, double x, double y, 
   return sqrt(bx * bx + by * by + bz * bz) / c + tx.t0;
 }
 
-// One accumulated term: gather the line of transmit row ROW at entry address a, interpolate at
-// ts, rotate by (pr, pi) and add.
+// Per-(receiver, voxel) geometry carried from one receiver-loop iteration to the next.
+struct Geo {
+  float rho2;       // lateral distance^2
+  float ep;         // excess path e - E0 [samples]
+  float mg;         // MAGIC + first table entry of the stage
+  float e0;         // E0 of the staged receiver
+  float pr, pi;     // receive phase factor (IQ); (1, 0) for RF
+  bool act;
+};
+
+// One accumulated term: gather the line of one transmit row at entry address a, interpolate at
+// ts, rotate by Prx and add.  IQ: three packed FP32x2 instructions (FFMA2, new on sm_100: one
+// issue slot for two lane-FMAs; the scalar operands ts, s.re, s.im are broadcast by the
+// instruction itself):   s = c + ts * slope ;  acc += s.re * (pr, pi) ;  acc += s.im * (-pi, pr).
 template <int MODE, int OFF>
-__device__ __forceinline__ void term(unsigned a, float ts, float pr, float pi, float& accR, float& accI) {
+__device__ __forceinline__ void term(unsigned a, float ts, float2 p1, float2 p2, float2& acc) {
   if constexpr (ModeTraits<MODE>::iq) {
     const float4 v = lds128<OFF>(a);                 // (c.re, c.im, slope.re, slope.im)
-    const float sre = fmaf(ts, v.z, v.x);
-    const float sim = fmaf(ts, v.w, v.y);
-    accR = fmaf(sre, pr, accR);
-    accR = fmaf(-sim, pi, accR);
-    accI = fmaf(sre, pi, accI);
-    accI = fmaf(sim, pr, accI);
+    const float2 sv = __ffma2_rn(make_float2(ts, ts), make_float2(v.z, v.w), make_float2(v.x, v.y));
+    acc = __ffma2_rn(make_float2(sv.x, sv.x), p1, acc);
+    acc = __ffma2_rn(make_float2(sv.y, sv.y), p2, acc);
   } else {
     const float2 v = lds64f<OFF>(a);                 // (c, slope)
-    accR += v.x;
-    accR = fmaf(ts, v.y, accR);
+    acc.x += v.x;
+    acc.x = fmaf(ts, v.y, acc.x);
+  }
+}
+
+// Part 1: wait for the stage, read its meta entry, classify the aperture (exactly inside the
+// guard band).  a2e / band carry "voxel outside the grid" and "no apodization" (see the caller).
+__device__ __forceinline__ void geo_test(Geo& g, unsigned tab_full0, unsigned meta0, unsigned slot, unsigned phase,
+                                         float x, float y, int iz, float a2e, float band,
+                                         const TiledDev& tp, const Params& P) {
+  mbar_wait(tab_full0 + 8 * slot, phase);
+  const float4 meta = lds128<0>(meta0 + 16 * slot);      // (ex, ey, E0, MAGIC + stage offset)
+  const float dx = x - meta.x, dy = y - meta.y;
+  g.rho2 = fmaf(dx, dx, dy * dy);
+  g.e0 = meta.z;
+  g.mg = meta.w;
+  const float lhs = tp.four_f2 * g.rho2;
+  g.act = lhs <= a2e;
+  if (fabsf(lhs - a2e) <= band) g.act = aperture_exact(x, y, meta.x, meta.y, P.zs, iz, tp.z_array, P.fnum);
+}
+// Part 2 (active lanes): excess path and receive phase.
+template <bool IQ>
+__device__ __forceinline__ void geo_finish(Geo& g, float a, float a2, const TiledDev& tp) {
+  const float s2 = g.rho2 + a2;
+  const float d = s2 * rsqrt_approx(s2);
+  const float e = (g.rho2 * tp.kappa_f) * rcp_approx(a + d);
+  g.ep = e - g.e0;
+  if (IQ) {
+    float cyc = tp.ratio_f * e;
+    cyc -= rintf(cyc);
+    const float ang = 6.283185307179586f * cyc;
+    g.pr = cos_approx(ang);
+    g.pi = sin_approx(ang);
+  } else {
+    g.pr = 1.f;
+    g.pi = 0.f;
   }
 }
 
@@ -302,12 +350,11 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
   reg_inc<kRegsConsumer>();
   const int wz = warp / (kWX * kWY), wy = (warp / kWX) % kWY, wx = warp % kWX;
   const int lx = lane % kLaneX, ly = lane / kLaneX;
-  const float kappa = (float)tp.kappa;
-  const float ratio = (float)tp.ratio;
-  // table address of entry index bits: (bits(u) << TSH) + base_adj, where bits(u) still holds
-  // the float exponent pattern of MAGIC; base_adj removes it (mod 2^32)
-  unsigned base_adj = smem_u32(&sm.tab[0][0]) - (kMagicBits << TSH);
-  asm volatile("mov.b32 %0, %0;" : "+r"(base_adj));     // opaque: keeps (bits << TSH) + base one LEA
+  // table address of an entry: (bits(u) << TSH) + base_adj, where bits(u) still holds the float
+  // exponent pattern of MAGIC; addr_bias (a kernel parameter) removes it mod 2^32
+  const unsigned base_adj = smem_u32(&sm.tab[0][0]) + tp.addr_bias;
+  const unsigned meta0 = smem_u32(&sm.meta_tab[0]);
+  unsigned slot = 0, phase = 0;          // table-ring position of this warp (same in all consumer warps)
 
   for (int tile_i = blockIdx.x; tile_i < tp.n_tiles; tile_i += gridDim.x) {
     const TileDesc td = tp.tiles[tile_i];
@@ -315,17 +362,24 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
     const int iy = td.iy0 + wy * kLaneY + ly;
     const int iz = td.iz0 + wz;
     const bool in_grid = ix < P.nx && iy < P.ny && iz < P.nz;
-    const float x = P.xs[min(ix, P.nx - 1)], y = P.ys[min(iy, P.ny - 1)], z = P.zs[min(iz, P.nz - 1)];
+    const int izc = min(iz, P.nz - 1);
+    const float x = P.xs[min(ix, P.nx - 1)], y = P.ys[min(iy, P.ny - 1)], z = P.zs[izc];
     const double a_d = (double)z - tp.z_array;
-    const float a = (float)a_d;
+    // pin(): values the receiver loop reads every iteration are routed through a shuffle so that
+    // ptxas keeps them in registers instead of rematerialising them (FP64 ops, select chains)
+    const float a = pin((float)a_d);
+    // aperture test  4 f#^2 rho^2 <= a^2  with everything that switches it off folded into the
+    // two thresholds: voxel outside the grid -> never active; no apodization -> always active
     const float a2 = a * a;
+    const float a2e = pin(!in_grid ? -1.f : (P.apod ? a2 : __int_as_float(0x7f800000)));
+    const float band = pin((in_grid && P.apod) ? kBand * a2 : -1.f);
     float out_re = 0.f, out_im = 0.f;
 
     for (int ch = 0; ch < tp.n_chunks; ++ch) {
       const int q0 = ch * QC;
       // ---- per-(q, n) part in FP64: reduced transmit delay and transmit phase -------------
       float2 Tf[QP];
-      float accR[2 * QP], accI[2 * QP];
+      float2 acc[2 * QP];
 #pragma unroll
       for (int j = 0; j < 2 * QP; ++j) {
         const int q = min(q0 + j, P.Q - 1);
@@ -338,38 +392,17 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
           cyc -= rint(cyc);
           sm.cyc[IQ ? j : 0][tid] = (float)cyc;          // read back by this thread only
         }
-        accR[j] = 0.f;
-        accI[j] = 0.f;
+        acc[j] = make_float2(0.f, 0.f);
       }
 
       // ---- receiver loop ---------------------------------------------------------------
-      for (int li = 0; li < td.list_cnt; ++li, ++seq) {
-        const unsigned slot = seq % kTabStages;
-        mbar_wait(tab_full0 + 8 * slot, (seq / kTabStages) & 1u);
-        const float4 meta = sm.meta_tab[slot];
-        const float dx = x - meta.x, dy = y - meta.y;
-        const float rho2 = fmaf(dx, dx, dy * dy);
-        bool act = in_grid;
-        if (P.apod) {
-          const float lhs = tp.four_f2 * rho2;
-          bool in = lhs <= a2;
-          if (fabsf(lhs - a2) <= kBand * a2) in = aperture_exact(x, y, meta.x, meta.y, a_d, P.fnum);
-          act = act && in;
-        }
-        if (act) {
-          const float s2 = rho2 + a2;
-          const float d = s2 * rsqrt_approx(s2);
-          const float e = (rho2 * kappa) * rcp_approx(a + d);
-          const float ep = e - meta.z;
-          float pr = 1.f, pi = 0.f;
-          if (IQ) {
-            float cyc = ratio * e;
-            cyc -= rintf(cyc);
-            const float ang = 6.283185307179586f * cyc;
-            pr = cos_approx(ang);
-            pi = sin_approx(ang);
-          }
-          const float2 ep2 = make_float2(ep, ep), mg2 = make_float2(meta.w, meta.w);
+      for (int li = 0; li < td.list_cnt; ++li) {
+        Geo g;
+        geo_test(g, tab_full0, meta0, slot, phase, x, y, izc, a2e, band, tp, P);
+        if (g.act) {
+          geo_finish<IQ>(g, a, a2, tp);
+          const float2 ep2 = make_float2(g.ep, g.ep), mg2 = make_float2(g.mg, g.mg);
+          const float2 p1 = make_float2(g.pr, g.pi), p2 = make_float2(-g.pi, g.pr);
           constexpr int kRow = W * TB;
 #pragma unroll
           for (int jp = 0; jp < QP; ++jp) {
@@ -380,8 +413,8 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
             // immediates: row offsets of transmit 2 jp and 2 jp + 1 inside a stage
             switch (jp) {
 #define DAS_CASE(JP) case JP: \
-              term<MODE, (2 * JP) * kRow>(a0, ts.x, pr, pi, accR[2 * jp], accI[2 * jp]); \
-              term<MODE, ((2 * JP + 1) % (QC > 1 ? QC : 1)) * kRow>(a1, ts.y, pr, pi, accR[2 * jp + 1], accI[2 * jp + 1]); break;
+              term<MODE, (2 * JP) * kRow>(a0, ts.x, p1, p2, acc[2 * jp]); \
+              term<MODE, ((2 * JP + 1) % (QC > 1 ? QC : 1)) * kRow>(a1, ts.y, p1, p2, acc[2 * jp + 1]); break;
               DAS_CASE(0) DAS_CASE(1) DAS_CASE(2) DAS_CASE(3) DAS_CASE(4) DAS_CASE(5) DAS_CASE(6) DAS_CASE(7)
 #undef DAS_CASE
               default: break;
@@ -390,6 +423,8 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(tab_empty0 + 8 * slot);
+        slot = (slot + 1) % kTabStages;
+        phase ^= (slot == 0);
       }
 
       // ---- fold this chunk: x += sum_q Ptx_q * acc_q ---------------------------------------
@@ -399,10 +434,10 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
           if (IQ) {
             const float ang = 6.283185307179586f * sm.cyc[IQ ? j : 0][tid];
             const float cs = cos_approx(ang), sn = sin_approx(ang);
-            out_re = fmaf(accR[j], cs, fmaf(-accI[j], sn, out_re));
-            out_im = fmaf(accR[j], sn, fmaf(accI[j], cs, out_im));
+            out_re = fmaf(acc[j].x, cs, fmaf(-acc[j].y, sn, out_re));
+            out_im = fmaf(acc[j].x, sn, fmaf(acc[j].y, cs, out_im));
           } else {
-            out_re += accR[j];
+            out_re += acc[j].x;
           }
         }
       }

@@ -167,6 +167,8 @@ TiledPlan* tiled_plan_create(const Params& P, const das_plan_desc_t& d, int devi
   dv.z_array = z_a; dv.kappa = kappa; dv.ratio = fc / fs;
   dv.phase0 = fc * t_start - std::floor(fc * t_start);
   dv.four_f2 = (float)(4.0 * fnum * fnum);
+  dv.kappa_f = (float)kappa; dv.ratio_f = (float)(fc / fs);
+  dv.addr_bias = 0u - (kMagicBits << (P.iq ? 4 : 3));
   if ((e = up(tp, tiles_sorted, &dv.tiles)) != cudaSuccess || (e = up(tp, k0_sorted, &dv.k0tile)) != cudaSuccess ||
       (e = up(tp, list, &dv.list)) != cudaSuccess) {
     *cuda_err = e; tiled_plan_destroy(tp); return nullptr;
