@@ -54,8 +54,12 @@ typedef enum { DAS_STORE_FP32 = 0, DAS_STORE_FP16 = 1 } das_storage_t;
 typedef enum {
   DAS_ALGO_AUTO = 0,     /* tiled kernel when the geometry allows it, else the general kernel */
   DAS_ALGO_GENERAL = 1,  /* one thread per voxel, any element positions / normals (Alg. 1 shape) */
-  DAS_ALGO_TILED = 2     /* voxel-tiled, shared-memory staged kernel; needs a planar array with
+  DAS_ALGO_TILED = 2,    /* voxel-tiled, shared-memory staged kernel; needs a planar array with
                             all normals (0,0,1); DAS_ERR_UNSUPPORTED otherwise */
+  DAS_ALGO_TC = 3        /* frame batch on the tensor cores (tcgen05, section 3.4 on
+                            the batch-inner layout of section 3.2): n_frames a multiple of 8 (of 64 above
+                            64), IQ data, fp16 storage, <= 16 transmits, planar array with normals
+                            (0,0,1); DAS_ERR_UNSUPPORTED otherwise.  AUTO picks it when it applies. */
 } das_algo_t;
 
 /* One transmit event (one "observation" q of the paper). */
@@ -84,7 +88,10 @@ typedef struct {
   int   storage;      /* das_storage_t: precision of the converted (device-layout) channel data */
   int   algo;         /* das_algo_t */
   int   device;       /* CUDA device ordinal */
-  int   n_frames;     /* reserved for a frame batch; must be 0 or 1 */
+  int   n_frames;     /* B, frames per call that share this geometry; 0 or 1 = one frame.
+                         With B > 1 das_convert / das_execute / das_beamform_host take B frames:
+                         raw [B][Q][M][K], output [B][nx][ny][nz]; every frame is beamformed exactly
+                         as a one-frame call would (DAS_ALGO_TC, else frame by frame). */
 } das_plan_desc_t;
 
 /* Validates *desc, uploads geometry and small derived tables to desc->device, chooses launch
@@ -92,14 +99,15 @@ typedef struct {
 das_status_t das_plan_create(const das_plan_desc_t* desc, das_plan_t** out_plan);
 das_status_t das_plan_destroy(das_plan_t* plan);            /* NULL is allowed */
 
-size_t das_raw_bytes(const das_plan_t* plan);        /* Q*M*K * (8 for IQ, 4 for RF)              */
+size_t das_raw_bytes(const das_plan_t* plan);        /* B*Q*M*K * (8 for IQ, 4 for RF)            */
 size_t das_converted_bytes(const das_plan_t* plan);  /* size of the buffer das_convert writes      */
-size_t das_output_bytes(const das_plan_t* plan);     /* nx*ny*nz * (8 for IQ, 4 for RF)            */
+size_t das_output_bytes(const das_plan_t* plan);     /* B*nx*ny*nz * (8 for IQ, 4 for RF)          */
 int    das_plan_algo(const das_plan_t* plan);        /* the das_algo_t actually selected           */
+int    das_plan_frames(const das_plan_t* plan);      /* B (>= 1)                                   */
 
 /* Layout transform + cast (the paper's permute-and-convert pre-pass).
- *   d_raw   device, [Q][M][K] complex64 (re,im interleaved) for IQ or float32 for RF,
- *           samples contiguous in k (the paper's layout with B = 1)
+ *   d_raw   device, [B][Q][M][K] complex64 (re,im interleaved) for IQ or float32 for RF,
+ *           samples contiguous in k (the paper's input layout)
  *   d_conv  device, das_converted_bytes() bytes, 16-byte aligned; written entirely
  *   scale   every sample is multiplied by it before the cast (1.0f = none); lets the caller
  *           keep fp16 storage inside its normal range
@@ -107,10 +115,10 @@ int    das_plan_algo(const das_plan_t* plan);        /* the das_algo_t actually 
 das_status_t das_convert(const das_plan_t* plan, const void* d_raw, void* d_conv, float scale,
                          void* stream);
 
-/* Beamform one volume.
+/* Beamform one volume per frame (B volumes).
  *   d_conv  device, produced by das_convert with this plan (or a plan with identical
  *           n_tx, n_elem, n_samples, data_kind and storage)
- *   d_out   device, das_output_bytes() bytes, [nx][ny][nz] with z fastest (C order), complex64
+ *   d_out   device, das_output_bytes() bytes, [B][nx][ny][nz] with z fastest (C order), complex64
  *           (IQ) or float32 (RF); overwritten, not accumulated into; 8-byte aligned */
 das_status_t das_execute(const das_plan_t* plan, const void* d_conv, void* d_out, void* stream);
 

@@ -26,11 +26,11 @@ OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_SIZE = range(6)
 TX_PLANE, TX_DIVERGING = 0, 1
 DATA_IQ, DATA_RF = 0, 1
 STORE_FP32, STORE_FP16 = 0, 1
-ALGO_AUTO, ALGO_GENERAL, ALGO_TILED = 0, 1, 2
+ALGO_AUTO, ALGO_GENERAL, ALGO_TILED, ALGO_TC = 0, 1, 2, 3
 
 # every symbol include/das.h declares (checked against the header by tests/test_abi.py)
 EXPORTS = ("das_plan_create", "das_plan_destroy", "das_raw_bytes", "das_converted_bytes",
-           "das_output_bytes", "das_plan_algo", "das_convert", "das_execute", "das_beamform_host",
+           "das_output_bytes", "das_plan_algo", "das_plan_frames", "das_convert", "das_execute", "das_beamform_host",
            "das_plan_count_work", "das_status_string", "das_last_error", "das_launch_count")
 
 
@@ -88,6 +88,8 @@ def load(build_if_missing: bool = True):
         getattr(lib, name).argtypes = [vp]
     lib.das_plan_algo.restype = ctypes.c_int
     lib.das_plan_algo.argtypes = [vp]
+    lib.das_plan_frames.restype = ctypes.c_int
+    lib.das_plan_frames.argtypes = [vp]
     lib.das_convert.restype = ctypes.c_int
     lib.das_convert.argtypes = [vp, vp, vp, ctypes.c_float, vp]
     lib.das_execute.restype = ctypes.c_int
@@ -166,12 +168,12 @@ class Plan:
         self.n_tx, self.n_elem, self.n_samples = len(tx_type), len(elem_pos), int(n_samples)
 
     @classmethod
-    def from_workload(cls, w, *, storage=STORE_FP32, algo=ALGO_AUTO, device=0):
+    def from_workload(cls, w, *, storage=STORE_FP32, algo=ALGO_AUTO, device=0, n_frames=0):
         """Plan for a ``workloads.Workload``-shaped object (duck-typed)."""
         return cls(w.elem_pos, w.tx_type, w.tx_v, w.tx_t0, w.xs, w.ys, w.zs, c=w.c, fc=w.fc, fs=w.fs,
                    t_start=w.t_start, f_number=w.f_number, n_samples=w.n_samples,
                    data_kind=w.data_kind, storage=storage, algo=algo, device=device,
-                   elem_dir=getattr(w, "elem_dir", None))
+                   elem_dir=getattr(w, "elem_dir", None), n_frames=n_frames)
 
     # sizes -------------------------------------------------------------------------------
     @property
@@ -189,6 +191,10 @@ class Plan:
     @property
     def algo(self) -> int:
         return int(self._lib.das_plan_algo(self._h))
+
+    @property
+    def frames(self) -> int:
+        return int(self._lib.das_plan_frames(self._h))
 
     # calls -------------------------------------------------------------------------------
     def convert(self, d_raw: int, d_conv: int, scale: float = 1.0, stream: int = 0):
@@ -228,8 +234,8 @@ class Plan:
 
 
 def beamform_torch(plan: Plan, raw, *, stream=None, conv=None, out=None):
-    """Convenience for tests/bench: ``raw`` is a CUDA torch tensor holding [Q,M,K] complex64 (IQ)
-    or float32 (RF).  Allocates (or reuses) the converted and output tensors with torch, then
+    """Convenience for tests/bench: ``raw`` is a CUDA torch tensor holding [Q,M,K] (one frame) or
+    [B,Q,M,K] (a plan with n_frames = B) complex64 (IQ) or float32 (RF).  Allocates (or reuses) the converted and output tensors with torch, then
     calls das_convert + das_execute with their raw pointers on torch's current stream."""
     import torch
     assert raw.is_cuda and raw.is_contiguous()
@@ -238,7 +244,8 @@ def beamform_torch(plan: Plan, raw, *, stream=None, conv=None, out=None):
         conv = torch.empty(plan.converted_bytes, dtype=torch.uint8, device=raw.device)
     if out is None:
         dt = torch.complex64 if plan.data_kind == DATA_IQ else torch.float32
-        out = torch.empty(plan.grid_shape, dtype=dt, device=raw.device)
+        shape = plan.grid_shape if plan.frames == 1 else (plan.frames,) + tuple(plan.grid_shape)
+        out = torch.empty(shape, dtype=dt, device=raw.device)
     plan.convert(raw.data_ptr(), conv.data_ptr(), 1.0, s.cuda_stream)
     plan.execute(conv.data_ptr(), out.data_ptr(), s.cuda_stream)
     return out, conv

@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "das_internal.cuh"
+#include "das_tc.cuh"
 
 namespace das {
 
@@ -56,6 +57,9 @@ struct das_plan {
   size_t raw_bytes = 0, conv_bytes = 0, out_bytes = 0;
   std::vector<void*> dev_allocs;          // geometry tables
   TiledPlan* tiled = nullptr;
+  TcPlan* tc = nullptr;
+  int frames = 1;                         // B
+  size_t raw1 = 0, conv1 = 0, out1 = 0;   // per-frame sizes (frame-by-frame path)
   // staging for das_beamform_host (lazy)
   void* st_raw = nullptr;
   void* st_conv = nullptr;
@@ -66,6 +70,7 @@ static void free_plan(das_plan* p) {
   if (!p) return;
   DeviceGuard g(p->device);
   if (p->tiled) tiled_plan_destroy(p->tiled);
+  if (p->tc) tc_plan_destroy(p->tc);
   for (void* d : p->dev_allocs) cudaFree(d);
   if (p->st_raw) cudaFree(p->st_raw);
   if (p->st_conv) cudaFree(p->st_conv);
@@ -127,8 +132,15 @@ das_status_t das_plan_create(const das_plan_desc_t* d, das_plan_t** out_plan) {
   if (!std::isfinite(d->f_number)) { set_err("f_number must be finite"); return DAS_ERR_INVALID_ARG; }
   if (d->data_kind != DAS_DATA_IQ && d->data_kind != DAS_DATA_RF) { set_err("unknown data_kind %d", d->data_kind); return DAS_ERR_UNSUPPORTED; }
   if (d->storage != DAS_STORE_FP32 && d->storage != DAS_STORE_FP16) { set_err("unknown storage %d", d->storage); return DAS_ERR_UNSUPPORTED; }
-  if (d->algo != DAS_ALGO_AUTO && d->algo != DAS_ALGO_GENERAL && d->algo != DAS_ALGO_TILED) { set_err("unknown algo %d", d->algo); return DAS_ERR_UNSUPPORTED; }
-  if (d->n_frames != 0 && d->n_frames != 1) { set_err("n_frames = %d: frame batches are not implemented (one frame per call)", d->n_frames); return DAS_ERR_UNSUPPORTED; }
+  if (d->algo != DAS_ALGO_AUTO && d->algo != DAS_ALGO_GENERAL && d->algo != DAS_ALGO_TILED && d->algo != DAS_ALGO_TC) { set_err("unknown algo %d", d->algo); return DAS_ERR_UNSUPPORTED; }
+  if (d->n_frames < 0 || d->n_frames > 4096) { set_err("n_frames = %d is outside [0, 4096]", d->n_frames); return DAS_ERR_INVALID_ARG; }
+  if (d->algo == DAS_ALGO_TC) {
+    const int B = d->n_frames;
+    if (B < 8 || B % 8 || (B > 64 && B % 64) || d->data_kind != DAS_DATA_IQ || d->storage != DAS_STORE_FP16 || d->n_tx > 16) {
+      set_err("DAS_ALGO_TC needs n_frames a multiple of 8 (of 64 above 64), IQ data, fp16 storage and <= 16 transmits");
+      return DAS_ERR_UNSUPPORTED;
+    }
+  }
   if (d->data_kind == DAS_DATA_RF && d->fc != 0.f) { set_err("fc must be 0 for RF data (no phase rotation)"); return DAS_ERR_INVALID_ARG; }
   if (!finite_all(d->elem_pos, 3LL * d->n_elem) || !finite_all(d->xs, d->nx) ||
       !finite_all(d->ys, d->ny) || !finite_all(d->zs, d->nz) ||
@@ -169,9 +181,13 @@ das_status_t das_plan_create(const das_plan_desc_t* d, das_plan_t** out_plan) {
   P.c = d->c; P.fc = d->fc; P.fs = d->fs; P.t_start = d->t_start; P.fnum = d->f_number;
   const size_t in_elem = P.iq ? 8 : 4;
   const size_t st_elem = (P.iq ? 2 : 1) * 2 * (P.fp16 ? 2 : 4);   // (mid, slope) entry
-  p->raw_bytes = (size_t)rows * P.K * in_elem;
-  p->conv_bytes = (size_t)rows * Kp * st_elem;
-  p->out_bytes = (size_t)N * in_elem;
+  p->frames = d->n_frames > 1 ? d->n_frames : 1;
+  p->raw1 = (size_t)rows * P.K * in_elem;
+  p->conv1 = (size_t)rows * Kp * st_elem;
+  p->out1 = (size_t)N * in_elem;
+  p->raw_bytes = p->raw1 * p->frames;
+  p->conv_bytes = p->conv1 * p->frames;
+  p->out_bytes = p->out1 * p->frames;
 
   DeviceGuard g(d->device);
   if (!g.ok) { das_status_t s = cuda_fail(g.err, "selecting the CUDA device"); delete p; return s; }
@@ -201,7 +217,24 @@ das_status_t das_plan_create(const das_plan_desc_t* d, das_plan_t** out_plan) {
   }
 
   p->algo = DAS_ALGO_GENERAL;
-  if (d->algo != DAS_ALGO_GENERAL) {
+  if (d->algo == DAS_ALGO_TC || (d->algo == DAS_ALGO_AUTO && p->frames > 1)) {
+    char why[256] = "";
+    cudaError_t ce = cudaSuccess;
+    p->tc = tc_plan_create(P, *d, p->frames, d->device, why, sizeof(why), &ce);
+    if (p->tc) {
+      p->algo = DAS_ALGO_TC;
+      p->conv_bytes = tc_converted_bytes(p->tc, P);
+    } else if (ce != cudaSuccess) {
+      das_status_t s = cuda_fail(ce, "building the tensor-core plan");
+      free_plan(p);
+      return s;
+    } else if (d->algo == DAS_ALGO_TC) {
+      set_err("tensor-core kernel not applicable: %s", why);
+      free_plan(p);
+      return DAS_ERR_UNSUPPORTED;
+    }
+  }
+  if (p->algo != DAS_ALGO_TC && d->algo != DAS_ALGO_GENERAL) {
     char why[256] = "";
     cudaError_t ce = cudaSuccess;
     p->tiled = tiled_plan_create(P, *d, d->device, why, sizeof(why), &ce);
@@ -230,6 +263,7 @@ size_t das_raw_bytes(const das_plan_t* p) { return p ? p->raw_bytes : 0; }
 size_t das_converted_bytes(const das_plan_t* p) { return p ? p->conv_bytes : 0; }
 size_t das_output_bytes(const das_plan_t* p) { return p ? p->out_bytes : 0; }
 int das_plan_algo(const das_plan_t* p) { return p ? p->algo : -1; }
+int das_plan_frames(const das_plan_t* p) { return p ? p->frames : 0; }
 
 das_status_t das_convert(const das_plan_t* p, const void* d_raw, void* d_conv, float scale, void* stream) {
   if (!p || !d_raw || !d_conv) { set_err("das_convert: NULL argument"); return DAS_ERR_INVALID_ARG; }
@@ -239,7 +273,14 @@ das_status_t das_convert(const das_plan_t* p, const void* d_raw, void* d_conv, f
   }
   DeviceGuard g(p->device);
   if (!g.ok) return cuda_fail(g.err, "selecting the CUDA device");
-  cudaError_t e = launch_convert(p->P, d_raw, d_conv, scale, static_cast<cudaStream_t>(stream));
+  cudaError_t e = cudaSuccess;
+  if (p->algo == DAS_ALGO_TC) {
+    e = launch_convert_batch(p->tc, p->P, d_raw, d_conv, scale, static_cast<cudaStream_t>(stream));
+  } else {
+    for (int b = 0; b < p->frames && e == cudaSuccess; ++b)
+      e = launch_convert(p->P, static_cast<const char*>(d_raw) + b * p->raw1, static_cast<char*>(d_conv) + b * p->conv1,
+                         scale, static_cast<cudaStream_t>(stream));
+  }
   if (e != cudaSuccess) return cuda_fail(e, "das_convert launch");
   return DAS_OK;
 }
@@ -251,12 +292,20 @@ das_status_t das_execute(const das_plan_t* p, const void* d_conv, void* d_out, v
   }
   DeviceGuard g(p->device);
   if (!g.ok) return cuda_fail(g.err, "selecting the CUDA device");
-  cudaError_t e;
-  if (p->algo == DAS_ALGO_TILED) {
-    int nl = 0;
-    e = launch_tiled(p->tiled, p->P, d_conv, d_out, static_cast<cudaStream_t>(stream), &nl);
+  cudaError_t e = cudaSuccess;
+  if (p->algo == DAS_ALGO_TC) {
+    e = launch_tc(p->tc, p->P, d_conv, d_out, static_cast<cudaStream_t>(stream));
   } else {
-    e = launch_general(p->P, d_conv, d_out, static_cast<cudaStream_t>(stream));
+    for (int b = 0; b < p->frames && e == cudaSuccess; ++b) {
+      const char* cv = static_cast<const char*>(d_conv) + b * p->conv1;
+      char* o = static_cast<char*>(d_out) + b * p->out1;
+      if (p->algo == DAS_ALGO_TILED) {
+        int nl = 0;
+        e = launch_tiled(p->tiled, p->P, cv, o, static_cast<cudaStream_t>(stream), &nl);
+      } else {
+        e = launch_general(p->P, cv, o, static_cast<cudaStream_t>(stream));
+      }
+    }
   }
   if (e != cudaSuccess) return cuda_fail(e, "das_execute launch");
   return DAS_OK;

@@ -1,0 +1,272 @@
+// Host side of the frame-batch tensor-core kernel (das_tc.cuh): applicability, voxel tiles,
+// per-tile receiver lists with per-group delay bounds, stage sizing, batch-inner convert kernel.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <numeric>
+#include <vector>
+
+#include "das_tc.cuh"
+
+namespace das {
+
+cudaError_t launch_tc_kernel(const TcDev& tp, const Params& P, const void* d_conv, void* d_out, int grid, size_t smem, cudaStream_t s);
+
+struct TcPlan {
+  TcDev dev{};
+  int grid = 1;
+  size_t smem = 0;
+  int n_frames = 0;
+  std::vector<void*> allocs;
+};
+
+void tc_plan_destroy(TcPlan* tp) {
+  if (!tp) return;
+  for (void* d : tp->allocs) cudaFree(d);
+  delete tp;
+}
+
+size_t tc_converted_bytes(const TcPlan* tp, const Params& P) {
+  return (size_t)tp->dev.n_chunks * P.M * P.Q * tp->dev.KBp * (size_t)(2 * tp->dev.Bc) * 16;
+}
+int tc_frames_per_chunk(const TcPlan* tp) { return tp->dev.Bc; }
+
+namespace {
+template <typename T>
+cudaError_t up(TcPlan* tp, const std::vector<T>& h, const T** d_out) {
+  void* d = nullptr;
+  cudaError_t e = cudaMalloc(&d, std::max<size_t>(h.size(), 1) * sizeof(T));
+  if (e != cudaSuccess) return e;
+  tp->allocs.push_back(d);
+  if (!h.empty()) e = cudaMemcpy(d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice);
+  *d_out = static_cast<const T*>(d);
+  return e;
+}
+inline double excess(double rho, double a) { return rho * rho / (a + std::sqrt(rho * rho + a * a)); }
+}  // namespace
+
+TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, int device, char* why,
+                       size_t why_len, cudaError_t* cuda_err) {
+  *cuda_err = cudaSuccess;
+  auto refuse = [&](const char* msg) -> TcPlan* { snprintf(why, why_len, "%s", msg); return nullptr; };
+  // ---- applicability ------------------------------------------------------------------------
+  if (!P.iq || !P.fp16) return refuse("the tensor-core path needs IQ data in fp16 storage");
+  if (d.n_tx > 16) return refuse("more than 16 transmits");
+  if (n_frames < 8 || n_frames % 8) return refuse("frame count is not a multiple of 8");
+  int Bc = n_frames;
+  if (n_frames > 64) { if (n_frames % 64) return refuse("frame count above 64 is not a multiple of 64"); Bc = 64; }
+  const double z_a = d.elem_pos[2];
+  for (int m = 0; m < d.n_elem; ++m)
+    if ((double)d.elem_pos[3 * m + 2] != z_a) return refuse("receivers are not in one plane z = const");
+  if (d.elem_dir)
+    for (int m = 0; m < d.n_elem; ++m)
+      if (d.elem_dir[3 * m] != 0.f || d.elem_dir[3 * m + 1] != 0.f || d.elem_dir[3 * m + 2] != 1.f)
+        return refuse("receiver normals are not all (0,0,1)");
+  for (int i = 0; i < d.nz; ++i)
+    if (!((double)d.zs[i] > z_a)) return refuse("a voxel plane is not in front of the array (z <= z_array)");
+
+  const double c = d.c, fs = d.fs, fc = d.fc, t_start = d.t_start, fnum = d.f_number;
+  const bool apod = fnum > 0.0;
+  const double kappa = fs / c;
+  const int Q = d.n_tx, M = d.n_elem;
+  const int ntx = (d.nx + kTcGX - 1) / kTcGX, nty = (d.ny + kTcGY - 1) / kTcGY, ntz = (d.nz + kTcG - 1) / kTcG;
+  const long long n_tiles_ll = (long long)ntx * nty * ntz;
+  if (n_tiles_ll > (1 << 22)) return refuse("too many tiles");
+  const int n_tiles = (int)n_tiles_ll;
+  const int Kb = (P.K + kTcBlk - 1) / kTcBlk;
+
+  std::vector<TcTile> tiles(n_tiles);
+  std::vector<int2> trange((size_t)n_tiles * kTcG * Q);
+  std::vector<int> tbase((size_t)n_tiles * Q);
+  std::vector<uint4> list;
+  std::vector<double> work(n_tiles, 0.0);
+  list.reserve((size_t)n_tiles * std::min(M, 512));
+  int stage_blocks = 2;
+  const double cone = apod ? 1.0 / (2.0 * fnum) : 0.0;
+
+  int t = 0;
+  for (int tz = 0; tz < ntz; ++tz)
+    for (int ty = 0; ty < nty; ++ty)
+      for (int txi = 0; txi < ntx; ++txi, ++t) {
+        TcTile& td = tiles[t];
+        td.ix0 = txi * kTcGX; td.iy0 = ty * kTcGY; td.iz0 = tz * kTcG;
+        const int ix1 = std::min(td.ix0 + kTcGX, d.nx), iy1 = std::min(td.iy0 + kTcGY, d.ny);
+        double xlo = 1e300, xhi = -1e300, ylo = 1e300, yhi = -1e300;
+        for (int i = td.ix0; i < ix1; ++i) { xlo = std::min(xlo, (double)d.xs[i]); xhi = std::max(xhi, (double)d.xs[i]); }
+        for (int i = td.iy0; i < iy1; ++i) { ylo = std::min(ylo, (double)d.ys[i]); yhi = std::max(yhi, (double)d.ys[i]); }
+        // ---- transmit part: exact min / max of T_q over the voxels of each group ------------
+        int tlo_tile[16];
+        for (int q = 0; q < Q; ++q) tlo_tile[q] = 0x7fffffff;
+        for (int g = 0; g < kTcG; ++g) {
+          const int iz = std::min(td.iz0 + g, d.nz - 1);
+          const double z = d.zs[iz], a = z - z_a;
+          for (int q = 0; q < Q; ++q) {
+            const das_transmit_t& tx = d.tx[q];
+            double lo = 1e300, hi = -1e300;
+            for (int i = td.ix0; i < ix1; ++i)
+              for (int j = td.iy0; j < iy1; ++j) {
+                const double x = d.xs[i], y = d.ys[j];
+                double tau;
+                if (tx.type == DAS_TX_PLANE) tau = (x * tx.v[0] + y * tx.v[1] + z * tx.v[2]) / c + tx.t0;
+                else tau = std::sqrt((x - tx.v[0]) * (x - tx.v[0]) + (y - tx.v[1]) * (y - tx.v[1]) + (z - tx.v[2]) * (z - tx.v[2])) / c + tx.t0;
+                const double T = (tau + a / c - t_start) * fs;
+                lo = std::min(lo, T); hi = std::max(hi, T);
+              }
+            if (!(std::fabs(lo) < 1e8 && std::fabs(hi) < 1e8)) return refuse("sample coordinate out of range");
+            const int l16 = (int)std::floor(16.0 * (lo - kTcMargin)), h16 = (int)std::ceil(16.0 * (hi + kTcMargin));
+            trange[((size_t)t * kTcG + g) * Q + q] = make_int2(l16, h16);
+            tlo_tile[q] = std::min(tlo_tile[q], l16);
+          }
+        }
+        for (int q = 0; q < Q; ++q) tbase[(size_t)t * Q + q] = ((tlo_tile[q] >> 4) >> 2) * 4;   // multiple of 4, <= every floor(T)
+        // ---- receiver part: list of receivers seen by any group, bounds of e per group --------
+        td.list_off = (int)list.size();
+        for (int m = 0; m < M; ++m) {
+          const double ex = d.elem_pos[3 * m], ey = d.elem_pos[3 * m + 1];
+          const double nx_ = std::max(std::max(xlo - ex, ex - xhi), 0.0), ny_ = std::max(std::max(ylo - ey, ey - yhi), 0.0);
+          const double fx = std::max(std::fabs(xlo - ex), std::fabs(xhi - ex)), fy = std::max(std::fabs(ylo - ey), std::fabs(yhi - ey));
+          const double rho_min = std::sqrt(nx_ * nx_ + ny_ * ny_), rho_max = std::sqrt(fx * fx + fy * fy);
+          unsigned er[kTcG];
+          bool any = false;
+          for (int g = 0; g < kTcG; ++g) {
+            er[g] = 0xFFFFFFFFu;
+            if (td.iz0 + g >= d.nz) continue;
+            const double a = (double)d.zs[td.iz0 + g] - z_a;
+            if (apod && rho_min > cone * a * (1.0 + 1e-5)) continue;                 // no voxel of the group sees m
+            const double r_hi = apod ? std::min(rho_max, cone * a * (1.0 + 1e-5)) : rho_max;
+            const double e_lo = excess(rho_min, a) * kappa - kTcMargin, e_hi = excess(r_hi, a) * kappa + kTcMargin;
+            const int l16 = std::max((int)std::floor(16.0 * e_lo), 0), h16 = (int)std::ceil(16.0 * e_hi);
+            if (h16 > 0xFFFE) return refuse("receive delay exceeds the 16-bit bound format");
+            er[g] = (unsigned)l16 | ((unsigned)h16 << 16);
+            any = true;
+          }
+          if (!any) continue;
+          list.push_back(make_uint4((unsigned)m, er[0], er[1], er[2]));
+          // stage size and row bounds for every transmit
+          for (int q = 0; q < Q; ++q) {
+            int wlo = 0x7fffffff, whi = -0x7fffffff;
+            for (int g = 0; g < kTcG; ++g) {
+              int lo;
+              const int nb = tc_block_range(trange[((size_t)t * kTcG + g) * Q + q], er[g], lo);
+              if (nb) { wlo = std::min(wlo, lo); whi = std::max(whi, lo + nb); work[t] += nb; }
+            }
+            if (whi > wlo) {
+              stage_blocks = std::max(stage_blocks, whi - wlo);
+              if (wlo < -kTcPadBlocks || whi > Kb + kTcPadBlocks) return refuse("a sample window leaves the zero-padded record");
+            }
+          }
+        }
+        td.list_cnt = (int)list.size() - td.list_off;
+      }
+  if (stage_blocks > kTcMaxStageBlocks) { snprintf(why, why_len, "sample window per tile (%d k-blocks) exceeds the stage capacity (%d)", stage_blocks, kTcMaxStageBlocks); return nullptr; }
+
+  // order tiles by decreasing work (static round-robin schedule over persistent CTAs)
+  std::vector<int> order(n_tiles);
+  std::iota(order.begin(), order.end(), 0);
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return work[a] > work[b]; });
+  std::vector<TcTile> tiles_s(n_tiles);
+  std::vector<int2> trange_s(trange.size());
+  std::vector<int> tbase_s(tbase.size());
+  for (int i = 0; i < n_tiles; ++i) {
+    tiles_s[i] = tiles[order[i]];
+    std::memcpy(&trange_s[(size_t)i * kTcG * Q], &trange[(size_t)order[i] * kTcG * Q], sizeof(int2) * kTcG * Q);
+    std::memcpy(&tbase_s[(size_t)i * Q], &tbase[(size_t)order[i] * Q], sizeof(int) * Q);
+  }
+
+  TcPlan* tp = new TcPlan();
+  tp->n_frames = n_frames;
+  cudaDeviceProp prop;
+  cudaError_t e = cudaGetDeviceProperties(&prop, device);
+  if (e != cudaSuccess) { *cuda_err = e; delete tp; return nullptr; }
+  TcDev& dv = tp->dev;
+  dv.n_tiles = n_tiles;
+  dv.Bc = Bc;
+  dv.n_chunks = n_frames / Bc;
+  dv.KBp = tc_kblocks(P.K);
+  dv.stage_blocks = stage_blocks;
+  dv.z_array = z_a; dv.kappa = kappa; dv.ratio = fc / fs;
+  dv.phase0 = fc * t_start - std::floor(fc * t_start);
+  dv.four_f2 = (float)(4.0 * fnum * fnum);
+  dv.kappa_f = (float)kappa; dv.ratio_f = (float)(fc / fs);
+  tp->smem = tc_smem_bytes(Bc, stage_blocks);
+  if (tp->smem > 200 * 1024) { delete tp; return refuse("stage ring does not fit in shared memory"); }
+  tp->grid = std::max(1, std::min(n_tiles * dv.n_chunks, prop.multiProcessorCount));
+  if ((e = up(tp, tiles_s, &dv.tiles)) != cudaSuccess || (e = up(tp, trange_s, &dv.trange)) != cudaSuccess ||
+      (e = up(tp, tbase_s, &dv.tbase)) != cudaSuccess || (e = up(tp, list, &dv.list)) != cudaSuccess) {
+    *cuda_err = e; tc_plan_destroy(tp); return nullptr;
+  }
+  return tp;
+}
+
+cudaError_t launch_tc(const TcPlan* tp, const Params& P, const void* d_conv, void* d_out, cudaStream_t s) {
+  count_launch();
+  return launch_tc_kernel(tp->dev, P, d_conv, d_out, tp->grid, tp->smem, s);
+}
+
+// ---- batch-inner layout transform + cast (PAPER.md:149 permute to batch-inner, :194-200 FP16) ----
+//   in : raw   [B][Q][M][K] complex64, samples contiguous in k (the paper's input layout)
+//   out: convb [chunk][M][Q][KBp][N = 2 Bc][8] FP16; k-block kb holds samples 4 (kb - kTcPadBlocks) + u,
+//        u = 0..3; column 2 b: (re, im) of frame b per sample; column 2 b + 1: (im, -re) = -j y;
+//        zero outside 0 <= k < K.
+// One CTA per (m, q, chunk): reads Bc rows of K samples (coalesced along k), transposes through
+// shared memory in pieces of 64 samples, writes 16-byte column entries (coalesced along columns).
+namespace {
+constexpr int kCbSamples = 64;      // samples per piece = 16 k-blocks
+
+__global__ void __launch_bounds__(256)
+convert_batch_kernel(const float2* __restrict__ raw, uint4* __restrict__ convb, int M, int Q, int K, int KBp,
+                     int Bc, int n_frames, float scale) {
+  extern __shared__ __align__(16) unsigned char cb_smem[];
+  unsigned* tile = reinterpret_cast<unsigned*>(cb_smem);          // [Bc][kCbSamples + 1] half2 (re, im)
+  const int q = blockIdx.x % Q, m = (blockIdx.x / Q) % M, chunk = blockIdx.x / (Q * M);
+  const int N = 2 * Bc;
+  uint4* row = convb + (((long long)chunk * M + m) * Q + q) * (long long)KBp * N;
+  const uint4 zero4 = make_uint4(0u, 0u, 0u, 0u);
+  const int Kb = (K + kTcBlk - 1) / kTcBlk;
+  // zero pads
+  for (int i = threadIdx.x; i < kTcPadBlocks * N; i += blockDim.x) {
+    row[i] = zero4;
+    row[(long long)(kTcPadBlocks + Kb) * N + i] = zero4;
+  }
+  for (int k0 = 0; k0 < K; k0 += kCbSamples) {
+    __syncthreads();
+    for (int i = threadIdx.x; i < Bc * kCbSamples; i += blockDim.x) {
+      const int b = i / kCbSamples, kk = i % kCbSamples, k = k0 + kk;
+      unsigned v = 0u;
+      if (k < K) {
+        const float2 s = raw[(((long long)(chunk * Bc + b) * Q + q) * M + m) * K + k];
+        const __half2 h = __floats2half2_rn(s.x * scale, s.y * scale);
+        v = *reinterpret_cast<const unsigned*>(&h);
+      }
+      tile[b * (kCbSamples + 1) + kk] = v;
+    }
+    __syncthreads();
+    const int nblk = min(kCbSamples / kTcBlk, Kb - k0 / kTcBlk);
+    for (int i = threadIdx.x; i < nblk * N; i += blockDim.x) {
+      const int col = i % N, kb = i / N, b = col >> 1;
+      unsigned w[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const unsigned v = tile[b * (kCbSamples + 1) + kb * kTcBlk + u];        // (re, im)
+        // odd column: (im, -re): swap halves, flip the sign of the new high half
+        w[u] = (col & 1) ? (((v >> 16) | (v << 16)) ^ 0x80000000u) : v;
+      }
+      row[(long long)(kTcPadBlocks + k0 / kTcBlk + kb) * N + col] = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+  }
+}
+}  // namespace
+
+cudaError_t launch_convert_batch(const TcPlan* tp, const Params& P, const void* d_raw, void* d_conv,
+                                 float scale, cudaStream_t s) {
+  const TcDev& dv = tp->dev;
+  const size_t smem = (size_t)dv.Bc * (kCbSamples + 1) * 4;
+  const long long blocks = (long long)dv.n_chunks * P.M * P.Q;
+  convert_batch_kernel<<<(unsigned)blocks, 256, smem, s>>>(static_cast<const float2*>(d_raw), static_cast<uint4*>(d_conv),
+                                                             P.M, P.Q, P.K, dv.KBp, dv.Bc, tp->n_frames, scale);
+  count_launch();
+  return cudaGetLastError();
+}
+
+}  // namespace das

@@ -52,7 +52,9 @@ def _good_kwargs():
     (dict(storage=3), "UNSUPPORTED"),
     (dict(data_kind=2), "UNSUPPORTED"),
     (dict(algo=9), "UNSUPPORTED"),
-    (dict(n_frames=4), "UNSUPPORTED"),
+    (dict(n_frames=-1), "INVALID_ARG"),
+    (dict(n_frames=4, algo=3, storage=1), "UNSUPPORTED"),      # tensor-core batch needs a multiple of 8
+    (dict(n_frames=8, algo=3, storage=0), "UNSUPPORTED"),      # ... and fp16 storage
     (dict(xs=[float("inf")]), "INVALID_ARG"),
     (dict(elem_dir=np.tile([0, 0, 2.0], (4, 1))), "INVALID_ARG"),
 ])
