@@ -5,6 +5,12 @@ namespace das {
 
 namespace {
 
+// (k-block count, first k-block) of one (q, m) item for one voxel group, packed so that one
+// shuffle hands it from the lane that computed it (lane = q) to the whole warp
+__device__ __forceinline__ int pack_range(int nb, int lo) { return (lo << 8) | nb; }
+__device__ __forceinline__ int range_nb(int pk) { return pk & 0xff; }
+__device__ __forceinline__ int range_lo(int pk) { return pk >> 8; }
+
 // Work items: (chunk, tile), tile fastest; every warp role walks the same sequence.
 __global__ void __launch_bounds__(kTcThreads, 1)
 tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ convb, float2* __restrict__ out) {
@@ -18,15 +24,16 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
   const int n_work = tp.n_tiles * tp.n_chunks;
   const long long n_vox = (long long)P.nx * P.ny * P.nz;
   const long long chunk_bytes = (long long)P.M * P.Q * tp.KBp * slab;
+  const int ql = min(lane & 15, P.Q - 1);                    // the transmit this lane computes ranges for
 
   const unsigned b_full0 = smem_u32(&sm.b_full[0]), b_empty0 = smem_u32(&sm.b_empty[0]);
   const unsigned a_full0 = smem_u32(&sm.a_full[0][0]), a_empty0 = smem_u32(&sm.a_empty[0][0]);
   const unsigned d_full = smem_u32(&sm.d_full), d_empty = smem_u32(&sm.d_empty);
 
   if (tid == 0) {
-    for (int s = 0; s < kTcStages; ++s) { mbar_init(b_full0 + 8 * s, 1); mbar_init(b_empty0 + 8 * s, 1); }
-    for (int i = 0; i < 2 * kTcG; ++i) { mbar_init(a_full0 + 8 * i, 4); mbar_init(a_empty0 + 8 * i, 1); }
-    mbar_init(d_full, 1);
+    for (int s = 0; s < kTcStages; ++s) { mbar_init(b_full0 + 8 * s, 1); mbar_init(b_empty0 + 8 * s, kTcG); }
+    for (int i = 0; i < kTcABufs * kTcG; ++i) { mbar_init(a_full0 + 8 * i, 4); mbar_init(a_empty0 + 8 * i, 1); }
+    mbar_init(d_full, kTcG);
     mbar_init(d_empty, kTcGenWarps);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -35,87 +42,99 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
   __syncthreads();
   tc_fence_after();
   const unsigned tmem = sm.tmem_base;
-  // TMEM columns: D of group g at g * N; A buffer (g, buf) at kTcG * N + (2 g + buf) * kTcACols
+  // TMEM columns: D of group g at g * N; A buffer (g, buf) at kTcG * N + (kTcABufs g + buf) * kTcACols
   const unsigned a_col0 = (unsigned)(kTcG * N);
 
   if (warp == kTcGenWarps) {
     // ===================================== TMA PRODUCER =======================================
-    if (lane == 0) {
-      unsigned it = 0;
-      for (int work = blockIdx.x; work < n_work; work += gridDim.x) {
-        const int tile_i = work % tp.n_tiles, chunk = work / tp.n_tiles;
-        const TcTile td = tp.tiles[tile_i];
-        const unsigned char* base = convb + (long long)chunk * chunk_bytes;
-        for (int li = 0; li < td.list_cnt; ++li) {
-          const uint4 ent = __ldg(&tp.list[td.list_off + li]);
-          const int m = (int)ent.x;
-          const unsigned er[kTcG] = {ent.y, ent.z, ent.w};
-          for (int q = 0; q < P.Q; ++q, ++it) {
-            int wlo = 0x7fffffff, whi = -0x7fffffff;
+    // lane q works out the window of item (q, m); lane 0 issues the copies in item order
+    unsigned it = 0;
+    for (int work = blockIdx.x; work < n_work; work += gridDim.x) {
+      const int tile_i = work % tp.n_tiles, chunk = work / tp.n_tiles;
+      const TcTile td = tp.tiles[tile_i];
+      const unsigned char* base = convb + (long long)chunk * chunk_bytes;
+      int2 tr[kTcG];
 #pragma unroll
-            for (int g = 0; g < kTcG; ++g) {
-              int lo;
-              const int nb = tc_block_range(__ldg(&tp.trange[((long long)tile_i * kTcG + g) * P.Q + q]), er[g], lo);
-              if (nb) { wlo = min(wlo, lo); whi = max(whi, lo + nb); }
-            }
+      for (int g = 0; g < kTcG; ++g) tr[g] = __ldg(&tp.trange[((long long)tile_i * kTcG + g) * P.Q + ql]);
+      uint4 ent = td.list_cnt ? __ldg(&tp.list[td.list_off]) : make_uint4(0, 0, 0, 0);
+      for (int li = 0; li < td.list_cnt; ++li) {
+        const uint4 cur = ent;
+        if (li + 1 < td.list_cnt) ent = __ldg(&tp.list[td.list_off + li + 1]);
+        const unsigned er[kTcG] = {cur.y, cur.z, cur.w};
+        int wlo = 0x7fffffff, whi = -0x7fffffff;
+#pragma unroll
+        for (int g = 0; g < kTcG; ++g) {
+          int lo;
+          const int nb = tc_block_range(tr[g], er[g], lo);
+          if (nb) { wlo = min(wlo, lo); whi = max(whi, lo + nb); }
+        }
+        if (whi <= wlo) { wlo = 0; whi = 0; }
+        const long long row0 = (long long)cur.x * P.Q * tp.KBp + kTcPadBlocks;
+        for (int q = 0; q < P.Q; ++q, ++it) {
+          const int wlo_q = __shfl_sync(0xffffffffu, wlo, q), whi_q = __shfl_sync(0xffffffffu, whi, q);
+          if (lane == 0) {
             const unsigned s = it % kTcStages;
             mbar_wait(b_empty0 + 8 * s, ((it / kTcStages) & 1u) ^ 1u);
-            if (whi <= wlo) { wlo = 0; whi = 0; }
-            sm.wlo[s] = wlo;
-            const unsigned bytes = (unsigned)(whi - wlo) * slab;
+            sm.wlo[s] = wlo_q;
+            const unsigned bytes = (unsigned)(whi_q - wlo_q) * slab;
             if (bytes) {
               mbar_arrive_expect_tx(b_full0 + 8 * s, bytes);
-              const unsigned char* src = base + (((long long)m * P.Q + q) * tp.KBp + kTcPadBlocks + wlo) * (long long)slab;
-              tma_bulk_g2s(stage0 + s * stage_bytes, src, bytes, b_full0 + 8 * s);
+              tma_bulk_g2s(stage0 + s * stage_bytes, base + (row0 + (long long)q * tp.KBp + wlo_q) * (long long)slab, bytes, b_full0 + 8 * s);
             } else {
               mbar_arrive(b_full0 + 8 * s);
             }
           }
+          __syncwarp();
         }
       }
     }
-  } else if (warp == kTcGenWarps + 1) {
-    // ===================================== MMA ISSUER =========================================
-    if (lane == 0) {
-      const unsigned idesc = tc_idesc(N);
-      unsigned it = 0, a_it[kTcG] = {0, 0, 0}, n_done = 0;
-      for (int work = blockIdx.x; work < n_work; work += gridDim.x, ++n_done) {
-        const int tile_i = work % tp.n_tiles;
-        const TcTile td = tp.tiles[tile_i];
+  } else if (warp > kTcGenWarps) {
+    // ===================================== MMA ISSUERS ========================================
+    // one warp per voxel group; lane q works out the k-block range of item (q, m), lane 0 issues
+    const int g = warp - kTcGenWarps - 1;
+    const unsigned idesc = tc_idesc(N);
+    const unsigned d_tmem = tmem + (unsigned)(g * N);
+    const unsigned a_tmem0 = tmem + a_col0 + (unsigned)(kTcABufs * g) * kTcACols;
+    unsigned it = 0, a_it = 0, n_done = 0;
+    for (int work = blockIdx.x; work < n_work; work += gridDim.x, ++n_done) {
+      const int tile_i = work % tp.n_tiles;
+      const TcTile td = tp.tiles[tile_i];
+      const int2 tr = __ldg(&tp.trange[((long long)tile_i * kTcG + g) * P.Q + ql]);
+      if (lane == 0) {
         mbar_wait(d_empty, (n_done & 1u) ^ 1u);            // epilogue of the previous tile has drained D
         tc_fence_after();
-        unsigned acc[kTcG] = {0, 0, 0};
-        for (int li = 0; li < td.list_cnt; ++li) {
-          const uint4 ent = __ldg(&tp.list[td.list_off + li]);
-          const unsigned er[kTcG] = {ent.y, ent.z, ent.w};
-          for (int q = 0; q < P.Q; ++q, ++it) {
-            const unsigned s = it % kTcStages;
-            mbar_wait(b_full0 + 8 * s, (it / kTcStages) & 1u);
-            const int wlo = sm.wlo[s];
-            const unsigned sbase = stage0 + s * stage_bytes;
-#pragma unroll
-            for (int g = 0; g < kTcG; ++g) {
-              int lo;
-              const int nb = tc_block_range(__ldg(&tp.trange[((long long)tile_i * kTcG + g) * P.Q + q]), er[g], lo);
-              for (int p0 = 0; p0 < nb; p0 += kTcPassBlocks, ++a_it[g]) {
-                const unsigned buf = a_it[g] & 1u;
-                mbar_wait(a_full0 + 8 * (2 * g + buf), (a_it[g] >> 1) & 1u);
-                tc_fence_after();
-                const int nbp = min(kTcPassBlocks, nb - p0);
-                for (int j = 0; j < nbp / 2; ++j) {
-                  const unsigned baddr = sbase + (unsigned)(lo - wlo + p0 + 2 * j) * slab;
-                  tc_mma_ts(tmem + (unsigned)(g * N), tmem + a_col0 + (2 * g + buf) * kTcACols + 8 * j,
-                            tc_smem_desc(baddr, slab, 128), idesc, acc[g]);
-                  acc[g] = 1;
-                }
-                tc_commit(a_empty0 + 8 * (2 * g + buf));      // A buffer free once these MMAs have read it
-              }
-            }
-            tc_commit(b_empty0 + 8 * s);                      // stage free once its MMAs are done
-          }
-        }
-        tc_commit(d_full);                                    // all MMAs of the tile complete -> epilogue
       }
+      __syncwarp();
+      unsigned acc = 0;
+      uint4 ent = td.list_cnt ? __ldg(&tp.list[td.list_off]) : make_uint4(0, 0, 0, 0);
+      for (int li = 0; li < td.list_cnt; ++li) {
+        const uint4 cur = ent;
+        if (li + 1 < td.list_cnt) ent = __ldg(&tp.list[td.list_off + li + 1]);
+        int lo;
+        const int nb = tc_block_range(tr, g == 0 ? cur.y : (g == 1 ? cur.z : cur.w), lo);
+        const int pk = pack_range(nb, lo);
+        for (int q = 0; q < P.Q; ++q, ++it) {
+          const int pk_q = __shfl_sync(0xffffffffu, pk, q);
+          if (lane == 0) {
+            const unsigned s = it % kTcStages;
+            const int nb_q = range_nb(pk_q), lo_q = range_lo(pk_q);
+            mbar_wait(b_full0 + 8 * s, (it / kTcStages) & 1u);
+            const unsigned b0 = stage0 + s * stage_bytes + (unsigned)(lo_q - sm.wlo[s]) * slab;
+            for (int p0 = 0; p0 < nb_q; p0 += kTcPassBlocks, ++a_it) {
+              const unsigned buf = a_it % kTcABufs;
+              mbar_wait(a_full0 + 8 * (kTcABufs * g + buf), (a_it / kTcABufs) & 1u);
+              tc_fence_after();
+              tc_mma_ts(d_tmem, a_tmem0 + buf * kTcACols, tc_smem_desc(b0 + (unsigned)p0 * slab, slab, 128), idesc, acc);
+              acc = 1;
+              tc_commit(a_empty0 + 8 * (kTcABufs * g + buf));    // A buffer free once this MMA has read it
+            }
+            tc_commit(b_empty0 + 8 * s);                         // this group is done with the stage
+          }
+          __syncwarp();
+        }
+      }
+      if (lane == 0) tc_commit(d_full);                          // this group's MMAs of the tile are complete
+      __syncwarp();
     }
   } else {
     // ===================================== GENERATORS =========================================
@@ -124,7 +143,7 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
     const int lx = row % kTcGX, ly = row / kTcGX;
     const unsigned lane_base = ((unsigned)((warp & 3) * 32)) << 16;
     const unsigned d_addr = tmem + lane_base + (unsigned)(g * N);
-    const unsigned a_addr0 = tmem + lane_base + a_col0 + (unsigned)(2 * g) * kTcACols;
+    const unsigned a_addr0 = tmem + lane_base + a_col0 + (unsigned)(kTcABufs * g) * kTcACols;
     unsigned a_it = 0, n_done = 0;
 
     for (int work = blockIdx.x; work < n_work; work += gridDim.x, ++n_done) {
@@ -139,6 +158,8 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
       const float a2 = a * a;
       const float a2e = !in_grid ? -1.f : (P.apod ? a2 : __int_as_float(0x7f800000));
       const float band = (in_grid && P.apod) ? kBand * a2 : -1.f;
+      const int2 tr = __ldg(&tp.trange[((long long)tile_i * kTcG + g) * P.Q + ql]);   // this lane's transmit
+      const int tb_l = __ldg(&tp.tbase[(long long)tile_i * P.Q + ql]);
 
       // per-(q, n) part in FP64: reduced transmit delay and transmit phase factor
       float Tf[16], pc[16], ps[16];
@@ -155,11 +176,17 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
       }
       bool produced = false;
 
+      uint4 ent = td.list_cnt ? __ldg(&tp.list[td.list_off]) : make_uint4(0, 0, 0, 0);
       for (int li = 0; li < td.list_cnt; ++li) {
-        const uint4 ent = __ldg(&tp.list[td.list_off + li]);
-        const unsigned er = g == 0 ? ent.y : (g == 1 ? ent.z : ent.w);
+        const uint4 cur = ent;
+        if (li + 1 < td.list_cnt) ent = __ldg(&tp.list[td.list_off + li + 1]);
+        const unsigned er = g == 0 ? cur.y : (g == 1 ? cur.z : cur.w);
         if (er == 0xFFFFFFFFu) continue;                      // no voxel of this group sees receiver m
-        const float4 el = __ldg(&P.elem[ent.x]);
+        // k-block range of item (q = lane, m): number of blocks and slot offset  r = ki + roff
+        int lo;
+        const int nb_l = tc_block_range(tr, er, lo);
+        const int pk = pack_range(nb_l, tb_l - 4 * lo);
+        const float4 el = __ldg(&P.elem[cur.x]);
         // per-(m, n): aperture, excess path, receive phase (as in das_tiled.cuh)
         const float dx = x - el.x, dy = y - el.y;
         const float rho2 = fmaf(dx, dx, dy * dy);
@@ -173,42 +200,40 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
         cyc -= rintf(cyc);
         const float ang = 6.283185307179586f * cyc;
         const float pr = act ? cos_approx(ang) : 0.f, pi = act ? sin_approx(ang) : 0.f;
+        // reading A6 (term dropped unless 0 <= k <= K-2) as a window on ki + tbase_q: folded below
 
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
           if (q < P.Q) {
-            int lo;
-            const int nb = tc_block_range(__ldg(&tp.trange[((long long)tile_i * kTcG + g) * P.Q + q]), er, lo);
-            const int tb = __ldg(&tp.tbase[(long long)tile_i * P.Q + q]);
+            const int pk_q = __shfl_sync(0xffffffffu, pk, q);
+            const int tb_q = __shfl_sync(0xffffffffu, tb_l, q);
+            const int nb = range_nb(pk_q), roff = range_lo(pk_q);
             // fractional index: ki = floor(t) (round-to-nearest of t - 1/2), al = t - ki
             const float t = Tf[q] + e;
             const float u = (t - 0.5f) + kMagic;
             const int ki = (int)(__float_as_uint(u) - kMagicBits);
             const float al = t - (u - kMagic);
-            const bool valid = (unsigned)(ki + tb) <= (unsigned)(P.K - 2);       // reading A6
+            const bool valid = (unsigned)(ki + tb_q) <= (unsigned)(P.K - 2);
             // weights: P = Ptx_q Prx_m;  W1 = al P (sample k + 1),  W0 = P - W1 (sample k)
             const float wre = fmaf(pc[q], pr, -ps[q] * pi), wim = fmaf(pc[q], pi, ps[q] * pr);
             const float w1re = al * wre, w1im = al * wim;
             unsigned w0 = pack_half2(wre - w1re, w1im - wim);                    // (Re W0, -Im W0)
             unsigned w1 = pack_half2(w1re, -w1im);
             if (!valid) { w0 = 0u; w1 = 0u; }
-            const int r = ki + tb - 4 * lo;                   // slot of sample k inside the group's k-blocks
+            const int r = ki + roff;                          // slot of sample k inside the group's k-blocks
             for (int p0 = 0; p0 < nb; p0 += kTcPassBlocks, ++a_it) {
-              const unsigned buf = a_it & 1u;
-              mbar_wait(a_empty0 + 8 * (2 * g + buf), ((a_it >> 1) & 1u) ^ 1u);
-              tc_fence_after();
-              const int nbp = min(kTcPassBlocks, nb - p0);
-              for (int j = 0; j < nbp / 2; ++j) {
-                const int s0 = 4 * p0 + 8 * j;                // first slot of this MMA's K = 16
-                unsigned v[8];
+              const unsigned buf = a_it % kTcABufs;
+              const int rr = r - 4 * p0;                      // slot relative to this MMA's K = 16 (8 samples)
+              unsigned v[8];
 #pragma unroll
-                for (int i = 0; i < 8; ++i) v[i] = (r == s0 + i) ? w0 : ((r + 1 == s0 + i) ? w1 : 0u);
-                tmem_st8(a_addr0 + buf * kTcACols + 8 * j, v);
-              }
+              for (int i = 0; i < 8; ++i) v[i] = (rr == i) ? w0 : ((rr + 1 == i) ? w1 : 0u);
+              mbar_wait(a_empty0 + 8 * (kTcABufs * g + buf), ((a_it / kTcABufs) & 1u) ^ 1u);
+              tc_fence_after();
+              tmem_st8(a_addr0 + buf * kTcACols, v);
               tmem_wait_st();
               tc_fence_before();
               __syncwarp();
-              if (lane == 0) mbar_arrive(a_full0 + 8 * (2 * g + buf));
+              if (lane == 0) mbar_arrive(a_full0 + 8 * (kTcABufs * g + buf));
               produced = true;
             }
           }

@@ -29,8 +29,9 @@
 //                phase.  Per (q, m): fractional index, weights, the 8 packed FP16 pairs of an
 //                A row -> tcgen05.st.  After the last receiver: tcgen05.ld of D -> global.
 //   warp 12      TMA producer: one bulk copy per (q, m) of the k-blocks the tile needs.
-//   warp 13      MMA issuer (one thread): tcgen05.mma.kind::f16, A from TMEM, B from shared
-//                memory (K-major, no swizzle: a k-block of N columns x 16 B is one slab).
+//   warps 13..15 MMA issuers, one per voxel group (one thread each): tcgen05.mma.kind::f16,
+//                A from TMEM, B from shared memory (K-major, no swizzle: a k-block of
+//                N columns x 16 B is one slab), D of the group in TMEM.
 #pragma once
 
 #include "das_tiled.cuh"
@@ -41,14 +42,15 @@ constexpr int kTcGX = 16, kTcGY = 8;        // a voxel group: 16 x 8 lateral vox
 constexpr int kTcRows = kTcGX * kTcGY;      // = 128 = MMA M
 constexpr int kTcG = 3;                     // voxel groups (consecutive depths) per tile
 constexpr int kTcBlk = 4;                   // samples per k-block (8 FP16 = 16 B per column)
-constexpr int kTcPassBlocks = 4;            // k-blocks per pass: 2 MMAs of K = 16
+constexpr int kTcPassBlocks = 2;            // k-blocks per pass = one MMA of K = 16
+constexpr int kTcABufs = 4;                 // A ring per voxel group (TMEM), one MMA each
 constexpr int kTcStages = 4;                // shared-memory ring of staged sample windows
 constexpr int kTcPadBlocks = 16;            // zero k-blocks before and after every (m, q) row
 constexpr int kTcMaxStageBlocks = 16;       // largest window (k-blocks) one stage can hold
 constexpr int kTcGenWarps = 4 * kTcG;
-constexpr int kTcThreads = (kTcGenWarps + 2) * 32;
+constexpr int kTcThreads = (kTcGenWarps + 1 + kTcG) * 32;   // + TMA producer + one MMA issuer per group
 constexpr int kTcTmemCols = 512;
-constexpr int kTcACols = 16;                // TMEM columns of one A buffer (2 MMAs x 8 columns)
+constexpr int kTcACols = 8;                 // TMEM columns of one A buffer (K = 16 FP16 per row)
 constexpr float kTcMargin = 0.02f;          // samples: slack of the plan's delay bounds
 
 __host__ __device__ inline int tc_kblocks(int K) { return 2 * kTcPadBlocks + (K + kTcBlk - 1) / kTcBlk; }
@@ -136,7 +138,7 @@ __device__ __forceinline__ unsigned pack_half2(float lo, float hi) {
 
 struct alignas(128) TcSmemHeader {
   unsigned long long b_full[kTcStages], b_empty[kTcStages];
-  unsigned long long a_full[kTcG][2], a_empty[kTcG][2];
+  unsigned long long a_full[kTcG][kTcABufs], a_empty[kTcG][kTcABufs];
   unsigned long long d_full, d_empty;
   int wlo[kTcStages];                // first k-block of the staged window (producer -> MMA issuer)
   unsigned tmem_base;

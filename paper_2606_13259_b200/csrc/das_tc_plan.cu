@@ -161,10 +161,19 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
       }
   if (stage_blocks > kTcMaxStageBlocks) { snprintf(why, why_len, "sample window per tile (%d k-blocks) exceeds the stage capacity (%d)", stage_blocks, kTcMaxStageBlocks); return nullptr; }
 
-  // order tiles by decreasing work (static round-robin schedule over persistent CTAs)
+  // Tile order: depth slab by depth slab (heaviest slab first), all lateral tiles of a slab side by
+  // side.  The CTAs of a wave then walk the same receivers of the same depth at about the same
+  // time, so the sample windows one CTA pulls from HBM are found in L2 by its lateral neighbours
+  // (they overlap almost entirely); the cheap shallow slabs come last and level the tail.
+  std::vector<double> slab_work(ntz, 0.0);
+  for (int i = 0; i < n_tiles; ++i) slab_work[i / (ntx * nty)] += work[i];
   std::vector<int> order(n_tiles);
   std::iota(order.begin(), order.end(), 0);
-  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return work[a] > work[b]; });
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
+    const int sa = a / (ntx * nty), sb = b / (ntx * nty);
+    if (sa != sb) return slab_work[sa] > slab_work[sb];
+    return work[a] > work[b];
+  });
   std::vector<TcTile> tiles_s(n_tiles);
   std::vector<int2> trange_s(trange.size());
   std::vector<int> tbase_s(tbase.size());
