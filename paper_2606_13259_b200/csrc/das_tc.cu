@@ -144,7 +144,10 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
     const unsigned lane_base = ((unsigned)((warp & 3) * 32)) << 16;
     const unsigned d_addr = tmem + lane_base + (unsigned)(g * N);
     const unsigned a_addr0 = tmem + lane_base + a_col0 + (unsigned)(kTcABufs * g) * kTcACols;
+    const unsigned af0 = a_full0 + 8u * (unsigned)(kTcABufs * g), ae0 = a_empty0 + 8u * (unsigned)(kTcABufs * g);
+    const bool lane0 = lane == 0;
     unsigned a_it = 0, n_done = 0;
+    unsigned pend = 0;                                        // a_full barrier of the A tile whose store is in flight
 
     for (int work = blockIdx.x; work < n_work; work += gridDim.x, ++n_done) {
       const int tile_i = work % tp.n_tiles, chunk = work / tp.n_tiles;
@@ -200,44 +203,64 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
         cyc -= rintf(cyc);
         const float ang = 6.283185307179586f * cyc;
         const float pr = act ? cos_approx(ang) : 0.f, pi = act ? sin_approx(ang) : 0.f;
-        // reading A6 (term dropped unless 0 <= k <= K-2) as a window on ki + tbase_q: folded below
+        produced = true;
 
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
           if (q < P.Q) {
             const int pk_q = __shfl_sync(0xffffffffu, pk, q);
-            const int tb_q = __shfl_sync(0xffffffffu, tb_l, q);
-            const int nb = range_nb(pk_q), roff = range_lo(pk_q);
+            const int n_pass = range_nb(pk_q) >> 1;
             // fractional index: ki = floor(t) (round-to-nearest of t - 1/2), al = t - ki
             const float t = Tf[q] + e;
             const float u = (t - 0.5f) + kMagic;
-            const int ki = (int)(__float_as_uint(u) - kMagicBits);
             const float al = t - (u - kMagic);
-            const bool valid = (unsigned)(ki + tb_q) <= (unsigned)(P.K - 2);
+            // slot of sample k inside the item's k-blocks:  r = ki + (tbase_q - 4 lo)
+            int r = (int)__float_as_uint(u) + (range_lo(pk_q) - (int)kMagicBits);
             // weights: P = Ptx_q Prx_m;  W1 = al P (sample k + 1),  W0 = P - W1 (sample k)
             const float wre = fmaf(pc[q], pr, -ps[q] * pi), wim = fmaf(pc[q], pi, ps[q] * pr);
             const float w1re = al * wre, w1im = al * wim;
             unsigned w0 = pack_half2(wre - w1re, w1im - wim);                    // (Re W0, -Im W0)
             unsigned w1 = pack_half2(w1re, -w1im);
-            if (!valid) { w0 = 0u; w1 = 0u; }
-            const int r = ki + roff;                          // slot of sample k inside the group's k-blocks
-            for (int p0 = 0; p0 < nb; p0 += kTcPassBlocks, ++a_it) {
-              const unsigned buf = a_it % kTcABufs;
-              const int rr = r - 4 * p0;                      // slot relative to this MMA's K = 16 (8 samples)
+            if (td.edge) {
+              // reading A6: the term is dropped unless 0 <= k <= K-2 (a pad sample may not lend its
+              // neighbour a weight); only tiles whose windows touch the ends of the record get here
+              const int tb_q = __shfl_sync(0xffffffffu, tb_l, q);
+              const int ki = (int)(__float_as_uint(u) - kMagicBits);
+              if ((unsigned)(ki + tb_q) > (unsigned)(P.K - 2)) { w0 = 0u; w1 = 0u; }
+            }
+#pragma unroll 1
+            for (int p = 0; p < n_pass; ++p, r -= kTcBlk * kTcPassBlocks) {
+              // the A row of this MMA: slot r holds W0, slot r + 1 holds W1, every other slot 0
               unsigned v[8];
 #pragma unroll
-              for (int i = 0; i < 8; ++i) v[i] = (rr == i) ? w0 : ((rr + 1 == i) ? w1 : 0u);
-              mbar_wait(a_empty0 + 8 * (kTcABufs * g + buf), ((a_it / kTcABufs) & 1u) ^ 1u);
+              for (int i = 0; i < 8; ++i) v[i] = 0u;
+#pragma unroll
+              for (int i = -1; i < 8; ++i) {
+                const bool hit = r == i;
+                if (i >= 0) v[i] = hit ? w0 : v[i];
+                if (i < 7) v[i + 1] = hit ? w1 : v[i + 1];
+              }
+              const unsigned buf = a_it & (kTcABufs - 1);
+              // complete the previous A tile (its store has had the placement above to land)
+              if (pend) {
+                tmem_wait_st();
+                tc_fence_before();
+                if (lane0) mbar_arrive(pend);
+              }
+              mbar_wait(ae0 + 8u * buf, ((a_it / kTcABufs) & 1u) ^ 1u);
               tc_fence_after();
               tmem_st8(a_addr0 + buf * kTcACols, v);
-              tmem_wait_st();
-              tc_fence_before();
-              __syncwarp();
-              if (lane == 0) mbar_arrive(a_full0 + 8 * (kTcABufs * g + buf));
-              produced = true;
+              pend = af0 + 8u * buf;
+              ++a_it;
             }
           }
         }
+      }
+      if (pend) {
+        tmem_wait_st();
+        tc_fence_before();
+        if (lane0) mbar_arrive(pend);
+        pend = 0;
       }
 
       // ---- epilogue: D (FP32, TMEM) -> out[frame][voxel] -------------------------------------

@@ -43,7 +43,7 @@ constexpr int kTcRows = kTcGX * kTcGY;      // = 128 = MMA M
 constexpr int kTcG = 3;                     // voxel groups (consecutive depths) per tile
 constexpr int kTcBlk = 4;                   // samples per k-block (8 FP16 = 16 B per column)
 constexpr int kTcPassBlocks = 2;            // k-blocks per pass = one MMA of K = 16
-constexpr int kTcABufs = 4;                 // A ring per voxel group (TMEM), one MMA each
+constexpr int kTcABufs = 4;                 // A ring per voxel group (TMEM), one MMA each; power of two
 constexpr int kTcStages = 4;                // shared-memory ring of staged sample windows
 constexpr int kTcPadBlocks = 16;            // zero k-blocks before and after every (m, q) row
 constexpr int kTcMaxStageBlocks = 16;       // largest window (k-blocks) one stage can hold
@@ -58,6 +58,7 @@ __host__ __device__ inline int tc_kblocks(int K) { return 2 * kTcPadBlocks + (K 
 struct TcTile {
   int ix0, iy0, iz0;
   int list_off, list_cnt;
+  int edge;                    // 1 if a staged window touches sample 0 or K-1: the A6 rule needs the explicit test
 };
 
 struct TcDev {

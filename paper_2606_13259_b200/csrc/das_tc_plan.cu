@@ -91,6 +91,7 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
       for (int txi = 0; txi < ntx; ++txi, ++t) {
         TcTile& td = tiles[t];
         td.ix0 = txi * kTcGX; td.iy0 = ty * kTcGY; td.iz0 = tz * kTcG;
+        td.edge = 0;
         const int ix1 = std::min(td.ix0 + kTcGX, d.nx), iy1 = std::min(td.iy0 + kTcGY, d.ny);
         double xlo = 1e300, xhi = -1e300, ylo = 1e300, yhi = -1e300;
         for (int i = td.ix0; i < ix1; ++i) { xlo = std::min(xlo, (double)d.xs[i]); xhi = std::max(xhi, (double)d.xs[i]); }
@@ -154,6 +155,7 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
             if (whi > wlo) {
               stage_blocks = std::max(stage_blocks, whi - wlo);
               if (wlo < -kTcPadBlocks || whi > Kb + kTcPadBlocks) return refuse("a sample window leaves the zero-padded record");
+              if (kTcBlk * wlo <= 0 || kTcBlk * whi >= P.K - 1) td.edge = 1;
             }
           }
         }
