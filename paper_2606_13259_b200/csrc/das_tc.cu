@@ -1,19 +1,22 @@
 // Frame-batch tensor-core delay-and-sum kernel (tcgen05 / TMEM); design notes in das_tc.cuh.
+#include <climits>
+#include <cstdlib>
+
 #include "das_tc.cuh"
 
 namespace das {
 
 namespace {
 
-// (k-block count, first k-block) of one (q, m) item for one voxel group, packed so that one
-// shuffle hands it from the lane that computed it (lane = q) to the whole warp
-__device__ __forceinline__ int pack_range(int nb, int lo) { return (lo << 8) | nb; }
-__device__ __forceinline__ int range_nb(int pk) { return pk & 0xff; }
-__device__ __forceinline__ int range_lo(int pk) { return pk >> 8; }
+// (first k-block, passes) of one (q, m) item for one voxel group, packed so that one shuffle hands
+// it from the lane that worked it out (lane = q) to the whole warp
+__device__ __forceinline__ int pack_item(int blk, int n_pass) { return (blk << 2) | n_pass; }
+__device__ __forceinline__ int item_passes(int pk) { return pk & 3; }
+__device__ __forceinline__ int item_blk(int pk) { return pk >> 2; }
 
 // Work items: (chunk, tile), tile fastest; every warp role walks the same sequence.
 __global__ void __launch_bounds__(kTcThreads, 1)
-tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ convb, float2* __restrict__ out) {
+tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ convb, float2* __restrict__ out, const int dbg) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   TcSmemHeader& sm = *reinterpret_cast<TcSmemHeader*>(smem_raw);
   const unsigned stage0 = (smem_u32(smem_raw) + (unsigned)sizeof(TcSmemHeader) + 127u) & ~127u;
@@ -24,17 +27,18 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
   const int n_work = tp.n_tiles * tp.n_chunks;
   const long long n_vox = (long long)P.nx * P.ny * P.nz;
   const long long chunk_bytes = (long long)P.M * P.Q * tp.KBp * slab;
-  const int ql = min(lane & 15, P.Q - 1);                    // the transmit this lane computes ranges for
+  const int ql = min(lane & 15, P.Q - 1);                    // the transmit this lane reads windows for
 
   const unsigned b_full0 = smem_u32(&sm.b_full[0]), b_empty0 = smem_u32(&sm.b_empty[0]);
-  const unsigned a_full0 = smem_u32(&sm.a_full[0][0]), a_empty0 = smem_u32(&sm.a_empty[0][0]);
+  const unsigned a_full0 = smem_u32(&sm.a_full[0]), a_empty0 = smem_u32(&sm.a_empty[0]);
   const unsigned d_full = smem_u32(&sm.d_full), d_empty = smem_u32(&sm.d_empty);
 
   if (tid == 0) {
-    for (int s = 0; s < kTcStages; ++s) { mbar_init(b_full0 + 8 * s, 1); mbar_init(b_empty0 + 8 * s, kTcG); }
-    for (int i = 0; i < kTcABufs * kTcG; ++i) { mbar_init(a_full0 + 8 * i, 4); mbar_init(a_empty0 + 8 * i, 1); }
+    for (int s = 0; s < kTcMaxStages; ++s) { mbar_init(b_full0 + 8 * s, 1); mbar_init(b_empty0 + 8 * s, kTcG); }
+    for (int i = 0; i < kTcMaxABufs * kTcG; ++i) { mbar_init(a_full0 + 8 * i, 4); mbar_init(a_empty0 + 8 * i, 1); }
     mbar_init(d_full, kTcG);
     mbar_init(d_empty, kTcGenWarps);
+    mbar_init(smem_u32(&sm.sink), 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == kTcGenWarps) tmem_alloc(smem_u32(&sm.tmem_base), kTcTmemCols);
@@ -42,237 +46,243 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
   __syncthreads();
   tc_fence_after();
   const unsigned tmem = sm.tmem_base;
-  // TMEM columns: D of group g at g * N; A buffer (g, buf) at kTcG * N + (kTcABufs g + buf) * kTcACols
+  // TMEM columns: D of group g at g * N; A buffer (g, buf) at kTcG * N + (a_bufs g + buf) * kTcACols
   const unsigned a_col0 = (unsigned)(kTcG * N);
+  const unsigned nab = (unsigned)tp.a_bufs, nab_sh = (unsigned)tp.a_shift;   // A ring depth (power of two)
 
   if (warp == kTcGenWarps) {
     // ===================================== TMA PRODUCER =======================================
-    // lane q works out the window of item (q, m); lane 0 issues the copies in item order
-    unsigned it = 0;
+    // lane q works out the window of item (q, m): the union over the voxel groups; lane 0 issues
+    unsigned s = 0, ph = 0;                                  // stage and its phase parity
     for (int work = blockIdx.x; work < n_work; work += gridDim.x) {
       const int tile_i = work % tp.n_tiles, chunk = work / tp.n_tiles;
       const TcTile td = tp.tiles[tile_i];
       const unsigned char* base = convb + (long long)chunk * chunk_bytes;
-      int2 tr[kTcG];
-#pragma unroll
-      for (int g = 0; g < kTcG; ++g) tr[g] = __ldg(&tp.trange[((long long)tile_i * kTcG + g) * P.Q + ql]);
-      uint4 ent = td.list_cnt ? __ldg(&tp.list[td.list_off]) : make_uint4(0, 0, 0, 0);
+      const int tb4 = __ldg(&tp.tbase[(long long)tile_i * P.Q + ql]) >> 2;       // k-block of tbase_q
       for (int li = 0; li < td.list_cnt; ++li) {
-        const uint4 cur = ent;
-        if (li + 1 < td.list_cnt) ent = __ldg(&tp.list[td.list_off + li + 1]);
-        const unsigned er[kTcG] = {cur.y, cur.z, cur.w};
-        int wlo = 0x7fffffff, whi = -0x7fffffff;
-#pragma unroll
-        for (int g = 0; g < kTcG; ++g) {
-          int lo;
-          const int nb = tc_block_range(tr[g], er[g], lo);
-          if (nb) { wlo = min(wlo, lo); whi = max(whi, lo + nb); }
-        }
-        if (whi <= wlo) { wlo = 0; whi = 0; }
-        const long long row0 = (long long)cur.x * P.Q * tp.KBp + kTcPadBlocks;
-        for (int q = 0; q < P.Q; ++q, ++it) {
-          const int wlo_q = __shfl_sync(0xffffffffu, wlo, q), whi_q = __shfl_sync(0xffffffffu, whi, q);
+        const long long e = td.list_off + li;
+        const uint2 hd = __ldg(&tp.list[e]);
+        if (!hd.y) continue;
+        int wlo, wn;
+        tc_union_window(tp.codes + e * kTcG * 16 + ql, wlo, wn);
+        // byte offset of the window inside the chunk and its length, per lane = q
+        const long long src_l = ((long long)hd.x * P.Q * tp.KBp + kTcPadBlocks + (long long)ql * tp.KBp + tb4 + wlo) * (long long)slab;
+        const unsigned bytes_l = (unsigned)wn * slab;
+        for (int q = 0; q < P.Q; ++q) {
+          const long long src = __shfl_sync(0xffffffffu, src_l, q);
+          const unsigned bytes = __shfl_sync(0xffffffffu, bytes_l, q);
           if (lane == 0) {
-            const unsigned s = it % kTcStages;
-            mbar_wait(b_empty0 + 8 * s, ((it / kTcStages) & 1u) ^ 1u);
-            sm.wlo[s] = wlo_q;
-            const unsigned bytes = (unsigned)(whi_q - wlo_q) * slab;
+            mbar_wait_park(b_empty0 + 8 * s, ph ^ 1u);
             if (bytes) {
               mbar_arrive_expect_tx(b_full0 + 8 * s, bytes);
-              tma_bulk_g2s(stage0 + s * stage_bytes, base + (row0 + (long long)q * tp.KBp + wlo_q) * (long long)slab, bytes, b_full0 + 8 * s);
+              tma_bulk_g2s(stage0 + s * stage_bytes, base + src, bytes, b_full0 + 8 * s);
             } else {
               mbar_arrive(b_full0 + 8 * s);
             }
           }
+          if (++s == (unsigned)tp.n_stages) { s = 0; ph ^= 1u; }
           __syncwarp();
         }
       }
     }
   } else if (warp > kTcGenWarps) {
     // ===================================== MMA ISSUERS ========================================
-    // one warp per voxel group; lane q works out the k-block range of item (q, m), lane 0 issues
+    // One warp per voxel group.  The issue loop is a serial chain (wait -> MMA -> commit), so it is
+    // kept as short as it can be: lane q prepares item (q, m) (passes, offset of the group's window
+    // inside the staged one), every lane runs the same scalar loop (no divergence, one shuffle per
+    // item), and only the tcgen05 instructions sit under an elected lane.
     const int g = warp - kTcGenWarps - 1;
     const unsigned idesc = tc_idesc(N);
     const unsigned d_tmem = tmem + (unsigned)(g * N);
-    const unsigned a_tmem0 = tmem + a_col0 + (unsigned)(kTcABufs * g) * kTcACols;
-    unsigned it = 0, a_it = 0, n_done = 0;
+    const unsigned a_tmem0 = tmem + a_col0 + (nab * (unsigned)g) * kTcACols;
+    const unsigned af0 = a_full0 + 8u * (nab * (unsigned)g), ae0 = a_empty0 + 8u * (nab * (unsigned)g);
+    // descriptor of a B tile at shared address 0: LBO = one slab (the two K chunks), SBO = 128 B
+    const unsigned long long desc0 = tc_smem_desc(0u, slab, 128);
+    unsigned s = 0, ph = 0, a_it = 0, n_done = 0;
     for (int work = blockIdx.x; work < n_work; work += gridDim.x, ++n_done) {
       const int tile_i = work % tp.n_tiles;
       const TcTile td = tp.tiles[tile_i];
-      const int2 tr = __ldg(&tp.trange[((long long)tile_i * kTcG + g) * P.Q + ql]);
-      if (lane == 0) {
-        mbar_wait(d_empty, (n_done & 1u) ^ 1u);            // epilogue of the previous tile has drained D
-        tc_fence_after();
-      }
-      __syncwarp();
+      mbar_wait_park(d_empty, (n_done & 1u) ^ 1u);             // epilogue of the previous tile has drained D
+      tc_fence_after();
       unsigned acc = 0;
-      uint4 ent = td.list_cnt ? __ldg(&tp.list[td.list_off]) : make_uint4(0, 0, 0, 0);
       for (int li = 0; li < td.list_cnt; ++li) {
-        const uint4 cur = ent;
-        if (li + 1 < td.list_cnt) ent = __ldg(&tp.list[td.list_off + li + 1]);
-        int lo;
-        const int nb = tc_block_range(tr, g == 0 ? cur.y : (g == 1 ? cur.z : cur.w), lo);
-        const int pk = pack_range(nb, lo);
-        for (int q = 0; q < P.Q; ++q, ++it) {
-          const int pk_q = __shfl_sync(0xffffffffu, pk, q);
-          if (lane == 0) {
-            const unsigned s = it % kTcStages;
-            const int nb_q = range_nb(pk_q), lo_q = range_lo(pk_q);
-            mbar_wait(b_full0 + 8 * s, (it / kTcStages) & 1u);
-            const unsigned b0 = stage0 + s * stage_bytes + (unsigned)(lo_q - sm.wlo[s]) * slab;
-            for (int p0 = 0; p0 < nb_q; p0 += kTcPassBlocks, ++a_it) {
-              const unsigned buf = a_it % kTcABufs;
-              mbar_wait(a_full0 + 8 * (kTcABufs * g + buf), (a_it / kTcABufs) & 1u);
+        const long long e = td.list_off + li;
+        const uint2 hd = __ldg(&tp.list[e]);
+        if (!hd.y) continue;
+        int wlo, wn;
+        tc_union_window(tp.codes + e * kTcG * 16 + ql, wlo, wn);
+        const unsigned c = __ldg(&tp.codes[(e * kTcG + g) * 16 + ql]);
+        // passes | 16-byte units from the start of the staged window to this group's window << 2
+        const unsigned info_l = (unsigned)code_passes(c) |
+                                ((code_passes(c) ? (unsigned)((code_start2(c) >> 1) - wlo) * (slab >> 4) : 0u) << 2);
+        for (int q = 0; q < P.Q; ++q) {
+          const unsigned info = __shfl_sync(0xffffffffu, info_l, q);
+          const int np = (int)(info & 3u);
+          mbar_wait_park(b_full0 + 8 * s, ph);                 // also keeps an idle group in step with the ring
+          if (np) {
+            unsigned long long desc = desc0 + (unsigned long long)(((stage0 + s * stage_bytes) >> 4) + (info >> 2));
+            for (int p = 0; p < np; ++p, ++a_it, desc += (unsigned long long)((kTcPassBlocks * slab) >> 4)) {
+              const unsigned buf = a_it & (nab - 1u);
+              mbar_wait_park(af0 + 8u * buf, (a_it >> nab_sh) & 1u);
               tc_fence_after();
-              tc_mma_ts(d_tmem, a_tmem0 + buf * kTcACols, tc_smem_desc(b0 + (unsigned)p0 * slab, slab, 128), idesc, acc);
+              if (tc_elect()) {
+                if (!(dbg & 1)) tc_mma_ts(d_tmem, a_tmem0 + buf * kTcACols, desc, idesc, acc);
+                tc_commit(ae0 + 8u * buf);                     // A buffer free once this MMA has read it
+              }
               acc = 1;
-              tc_commit(a_empty0 + 8 * (kTcABufs * g + buf));    // A buffer free once this MMA has read it
             }
-            tc_commit(b_empty0 + 8 * s);                         // this group is done with the stage
+            if (tc_elect()) tc_commit(b_empty0 + 8 * s);       // this group is done with the stage
+          } else if (lane == 0) {
+            mbar_arrive(b_empty0 + 8 * s);                     // nothing to read: release at once
           }
-          __syncwarp();
+          if (++s == (unsigned)tp.n_stages) { s = 0; ph ^= 1u; }
         }
       }
-      if (lane == 0) tc_commit(d_full);                          // this group's MMAs of the tile are complete
-      __syncwarp();
+      if (tc_elect()) tc_commit(d_full);                       // this group's MMAs of the tile are complete
     }
   } else {
     // ===================================== GENERATORS =========================================
-    const int g = warp >> 2;                                  // voxel group = depth inside the tile
-    const int row = (warp & 3) * 32 + lane;                   // MMA row = TMEM lane
-    const int lx = row % kTcGX, ly = row / kTcGX;
+    // Two warp sets per voxel group share the transmits (set h takes q = 2 j + h): twice the warps
+    // to hide the latencies of the per-pass chain (shuffle -> index -> weights -> placement -> store).
+    const int g = warp / (4 * kTcSets);                       // voxel group = depth inside the tile
+    const int h = (warp >> 2) % kTcSets;                      // this warp set takes the transmits q = kTcSets j + h
+    const int row = (warp & 3) * 32 + lane;                   // MMA row = TMEM lane (quarter warp % 4)
     const unsigned lane_base = ((unsigned)((warp & 3) * 32)) << 16;
     const unsigned d_addr = tmem + lane_base + (unsigned)(g * N);
-    const unsigned a_addr0 = tmem + lane_base + a_col0 + (unsigned)(kTcABufs * g) * kTcACols;
-    const unsigned af0 = a_full0 + 8u * (unsigned)(kTcABufs * g), ae0 = a_empty0 + 8u * (unsigned)(kTcABufs * g);
+    const unsigned a_addr0 = tmem + lane_base + a_col0 + (nab * (unsigned)g) * kTcACols;
+    const unsigned af0 = a_full0 + 8u * (nab * (unsigned)g), ae0 = a_empty0 + 8u * (nab * (unsigned)g);
     const bool lane0 = lane == 0;
+    const bool lane_has_q = (lane & 15) < P.Q;
+    // epilogue columns of this set: half of D each when a half is a whole number of 16-column loads
+    const bool split = kTcSets == 2 && (N % 32) == 0;
+    const int col_lo = split ? h * (N / 2) : 0, col_hi = split ? col_lo + N / 2 : (h == 0 ? N : 0);
     unsigned a_it = 0, n_done = 0;
-    unsigned pend = 0;                                        // a_full barrier of the A tile whose store is in flight
+    // a_full barrier of the A tile whose store is in flight; a sink nobody waits on while there is none
+    unsigned pend = smem_u32(&sm.sink);
 
     for (int work = blockIdx.x; work < n_work; work += gridDim.x, ++n_done) {
       const int tile_i = work % tp.n_tiles, chunk = work / tp.n_tiles;
       const TcTile td = tp.tiles[tile_i];
-      const int ix = td.ix0 + lx, iy = td.iy0 + ly, iz = td.iz0 + g;
-      const bool in_grid = ix < P.nx && iy < P.ny && iz < P.nz;
-      const int izc = min(iz, P.nz - 1);
-      const float x = P.xs[min(ix, P.nx - 1)], y = P.ys[min(iy, P.ny - 1)], z = P.zs[izc];
-      const double a_d = (double)z - tp.z_array;
-      const float a = (float)a_d;
-      const float a2 = a * a;
-      const float a2e = !in_grid ? -1.f : (P.apod ? a2 : __int_as_float(0x7f800000));
-      const float band = (in_grid && P.apod) ? kBand * a2 : -1.f;
-      const int2 tr = __ldg(&tp.trange[((long long)tile_i * kTcG + g) * P.Q + ql]);   // this lane's transmit
+      const TcVoxel vx = tc_voxel(tp, P, td, row, g);
       const int tb_l = __ldg(&tp.tbase[(long long)tile_i * P.Q + ql]);
 
-      // per-(q, n) part in FP64: reduced transmit delay and transmit phase factor
-      float Tf[16], pc[16], ps[16];
+      // per-(q, n) part in FP64: reduced transmit delay and transmit phase factor, q = 2 j + h
+      float Tf[kTcQPerSet], pc[kTcQPerSet], ps[kTcQPerSet];
 #pragma unroll
-      for (int q = 0; q < 16; ++q) {
-        const int qq = min(q, P.Q - 1);
-        const double T = (tx_delay(P.tx[qq], x, y, z, P.c) + a_d / P.c - P.t_start) * P.fs;
-        Tf[q] = (float)(T - (double)__ldg(&tp.tbase[(long long)tile_i * P.Q + qq]));
+      for (int j = 0; j < kTcQPerSet; ++j) {
+        const int qq = min(kTcSets * j + h, P.Q - 1);
+        const double T = tc_T(P, vx, qq);
+        Tf[j] = (float)(T - (double)__ldg(&tp.tbase[(long long)tile_i * P.Q + qq]));
         double cyc = tp.phase0 + tp.ratio * T;
         cyc -= rint(cyc);
         const float ang = 6.283185307179586f * (float)cyc;
-        pc[q] = cos_approx(ang);
-        ps[q] = sin_approx(ang);
+        pc[j] = cos_approx(ang);
+        ps[j] = sin_approx(ang);
       }
       bool produced = false;
 
-      uint4 ent = td.list_cnt ? __ldg(&tp.list[td.list_off]) : make_uint4(0, 0, 0, 0);
+      // the list entry one iteration ahead: header, this lane's window code, receiver position
+      uint2 hd_n = make_uint2(0u, 0u);
+      unsigned cl_n = 0u;
+      float4 el_n = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (td.list_cnt) {
+        hd_n = __ldg(&tp.list[td.list_off]);
+        cl_n = __ldg(&tp.codes[((long long)td.list_off * kTcG + g) * 16 + ql]);
+        el_n = __ldg(&P.elem[hd_n.x]);
+      }
       for (int li = 0; li < td.list_cnt; ++li) {
-        const uint4 cur = ent;
-        if (li + 1 < td.list_cnt) ent = __ldg(&tp.list[td.list_off + li + 1]);
-        const unsigned er = g == 0 ? cur.y : (g == 1 ? cur.z : cur.w);
-        if (er == 0xFFFFFFFFu) continue;                      // no voxel of this group sees receiver m
-        // k-block range of item (q = lane, m): number of blocks and slot offset  r = ki + roff
-        int lo;
-        const int nb_l = tc_block_range(tr, er, lo);
-        const int pk = pack_range(nb_l, tb_l - 4 * lo);
-        const float4 el = __ldg(&P.elem[cur.x]);
+        const uint2 hd = hd_n;
+        const unsigned cl = lane_has_q ? cl_n : 0u;           // window of item (q = lane, m); none beyond Q
+        const float4 el = el_n;
+        if (li + 1 < td.list_cnt) {
+          const long long e = td.list_off + li + 1;
+          hd_n = __ldg(&tp.list[e]);
+          cl_n = __ldg(&tp.codes[(e * kTcG + g) * 16 + ql]);
+          el_n = __ldg(&P.elem[hd_n.x]);
+        }
+        if (!((hd.y >> g) & 1u)) continue;                    // no voxel of this group sees receiver m
         // per-(m, n): aperture, excess path, receive phase (as in das_tiled.cuh)
-        const float dx = x - el.x, dy = y - el.y;
-        const float rho2 = fmaf(dx, dx, dy * dy);
-        const float lhs = tp.four_f2 * rho2;
-        bool act = lhs <= a2e;
-        if (fabsf(lhs - a2e) <= band) act = aperture_exact(x, y, el.x, el.y, P.zs, izc, tp.z_array, P.fnum);
-        const float s2 = rho2 + a2;
-        const float d = s2 * rsqrt_approx(s2);
-        const float e = (rho2 * tp.kappa_f) * rcp_approx(a + d);
-        float cyc = tp.ratio_f * e;
+        bool act;
+        const float ex = tc_excess(tp, P, vx, el, act);
+        float cyc = tp.ratio_f * ex;
         cyc -= rintf(cyc);
         const float ang = 6.283185307179586f * cyc;
         const float pr = act ? cos_approx(ang) : 0.f, pi = act ? sin_approx(ang) : 0.f;
         produced = true;
 
 #pragma unroll
-        for (int q = 0; q < 16; ++q) {
-          if (q < P.Q) {
-            const int pk_q = __shfl_sync(0xffffffffu, pk, q);
-            const int n_pass = range_nb(pk_q) >> 1;
-            // fractional index: ki = floor(t) (round-to-nearest of t - 1/2), al = t - ki
-            const float t = Tf[q] + e;
-            const float u = (t - 0.5f) + kMagic;
-            const float al = t - (u - kMagic);
-            // slot of sample k inside the item's k-blocks:  r = ki + (tbase_q - 4 lo)
-            int r = (int)__float_as_uint(u) + (range_lo(pk_q) - (int)kMagicBits);
-            // weights: P = Ptx_q Prx_m;  W1 = al P (sample k + 1),  W0 = P - W1 (sample k)
-            const float wre = fmaf(pc[q], pr, -ps[q] * pi), wim = fmaf(pc[q], pi, ps[q] * pr);
-            const float w1re = al * wre, w1im = al * wim;
-            unsigned w0 = pack_half2(wre - w1re, w1im - wim);                    // (Re W0, -Im W0)
-            unsigned w1 = pack_half2(w1re, -w1im);
-            if (td.edge) {
-              // reading A6: the term is dropped unless 0 <= k <= K-2 (a pad sample may not lend its
-              // neighbour a weight); only tiles whose windows touch the ends of the record get here
-              const int tb_q = __shfl_sync(0xffffffffu, tb_l, q);
-              const int ki = (int)(__float_as_uint(u) - kMagicBits);
-              if ((unsigned)(ki + tb_q) > (unsigned)(P.K - 2)) { w0 = 0u; w1 = 0u; }
-            }
-#pragma unroll 1
-            for (int p = 0; p < n_pass; ++p, r -= kTcBlk * kTcPassBlocks) {
-              // the A row of this MMA: slot r holds W0, slot r + 1 holds W1, every other slot 0
-              unsigned v[8];
-#pragma unroll
-              for (int i = 0; i < 8; ++i) v[i] = 0u;
-#pragma unroll
-              for (int i = -1; i < 8; ++i) {
-                const bool hit = r == i;
-                if (i >= 0) v[i] = hit ? w0 : v[i];
-                if (i < 7) v[i + 1] = hit ? w1 : v[i + 1];
-              }
-              const unsigned buf = a_it & (kTcABufs - 1);
-              // complete the previous A tile (its store has had the placement above to land)
-              if (pend) {
-                tmem_wait_st();
-                tc_fence_before();
-                if (lane0) mbar_arrive(pend);
-              }
-              mbar_wait(ae0 + 8u * buf, ((a_it / kTcABufs) & 1u) ^ 1u);
-              tc_fence_after();
-              tmem_st8(a_addr0 + buf * kTcACols, v);
-              pend = af0 + 8u * buf;
-              ++a_it;
-            }
+        for (int j = 0; j < kTcQPerSet; ++j) {
+          // items in transmit order; with two warp sets q = 2 j belongs to set 0 and q = 2 j + 1 to
+          // set 1, and the ring slots of the other set's item are counted, not written
+          unsigned c_q, c_e = 0u, c_o = 0u;
+          if (kTcSets == 2) {
+            c_e = __shfl_sync(0xffffffffu, cl, 2 * j); c_o = __shfl_sync(0xffffffffu, cl, 2 * j + 1);
+            c_q = h ? c_o : c_e;
+            a_it += h ? (unsigned)code_passes(c_e) : 0u;
+          } else {
+            c_q = __shfl_sync(0xffffffffu, cl, j);
           }
+          const int n_pass = code_passes(c_q);
+          // fractional index: ki = floor(t) (round-to-nearest of t - 1/2), al = t - ki
+          const float t = Tf[j] + ex;
+          const float u = (t - 0.5f) + kMagic;
+          const float al = t - (u - kMagic);
+          // slot of sample k inside the item's window:  r = ki - window start
+          int r = (int)__float_as_uint(u) - (int)(kMagicBits + 2u * (unsigned)code_start2(c_q));
+          // weights: P = Ptx_q Prx_m;  W1 = al P (sample k + 1),  W0 = P - W1 (sample k)
+          const float wre = fmaf(pc[j], pr, -ps[j] * pi), wim = fmaf(pc[j], pi, ps[j] * pr);
+          const float w1re = al * wre, w1im = al * wim;
+          unsigned w0 = pack_half2(wre - w1re, w1im - wim);                    // (Re W0, -Im W0)
+          unsigned w1 = pack_half2(w1re, -w1im);
+          if (td.edge) {
+            // reading A6: the term is dropped unless 0 <= k <= K-2 (a pad sample may not lend its
+            // neighbour a weight); only tiles whose windows touch the ends of the record get here
+            const int tb_q = __shfl_sync(0xffffffffu, tb_l, min(kTcSets * j + h, P.Q - 1));
+            const int ki = (int)(__float_as_uint(u) - kMagicBits);
+            if ((unsigned)(ki + tb_q) > (unsigned)(P.K - 2)) { w0 = 0u; w1 = 0u; }
+          }
+#pragma unroll 1
+          for (int p = 0; p < n_pass; ++p, r -= kTcBlk * kTcPassBlocks) {
+            // the A row of this MMA: slot r holds W0, slot r + 1 holds W1, every other slot 0
+            unsigned v[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) v[i] = 0u;
+            if (!(dbg & 2))
+#pragma unroll
+            for (int i = -1; i < 8; ++i) {
+              const bool hit = r == i;
+              if (i >= 0) v[i] = hit ? w0 : v[i];
+              if (i < 7) v[i + 1] = hit ? w1 : v[i + 1];
+            }
+            const unsigned buf = a_it & (nab - 1u);
+            // complete the previous A tile (its store has had the placement above to land)
+            if (!(dbg & 8)) tmem_wait_st();
+            tc_fence_before();
+            if (lane0) mbar_arrive(pend);
+            if (!(dbg & 32)) mbar_wait_park(ae0 + 8u * buf, ((a_it >> nab_sh) & 1u) ^ 1u);
+            tc_fence_after();
+            if (!(dbg & 16)) tmem_st8(a_addr0 + buf * kTcACols, v);
+            pend = af0 + 8u * buf;
+            ++a_it;
+          }
+          if (kTcSets == 2) a_it += h ? 0u : (unsigned)code_passes(c_o);
         }
       }
-      if (pend) {
-        tmem_wait_st();
-        tc_fence_before();
-        if (lane0) mbar_arrive(pend);
-        pend = 0;
-      }
+      tmem_wait_st();
+      tc_fence_before();
+      if (lane0) mbar_arrive(pend);
+      pend = smem_u32(&sm.sink);
 
       // ---- epilogue: D (FP32, TMEM) -> out[frame][voxel] -------------------------------------
-      mbar_wait(d_full, n_done & 1u);
+      mbar_wait_park(d_full, n_done & 1u);
       tc_fence_after();
-      const long long vox = ((long long)ix * P.ny + iy) * P.nz + iz;
+      const long long vox = ((long long)vx.ix * P.ny + vx.iy) * P.nz + vx.iz;
       float2* dst = out + (long long)chunk * tp.Bc * n_vox + vox;
-      for (int c0 = 0; c0 < N; c0 += 16) {
+      for (int c0 = col_lo; c0 < col_hi; c0 += 16) {
         float v[16];
         tmem_ld16(d_addr + (unsigned)c0, v);
         tmem_wait_ld();
-        if (in_grid) {
+        if (vx.in_grid) {
 #pragma unroll
           for (int i = 0; i < 8; ++i)
             dst[(long long)(c0 / 2 + i) * n_vox] = produced ? make_float2(v[2 * i], v[2 * i + 1]) : make_float2(0.f, 0.f);
@@ -290,7 +300,101 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
   if (warp == kTcGenWarps) tmem_dealloc(tmem, kTcTmemCols);
 }
 
+// ---- plan-time window kernel -------------------------------------------------------------------
+// One CTA per tile, thread = (voxel group, MMA row).  For every listed receiver m and transmit q
+// it takes the minimum and maximum of floor(t_qmn) over the ACTIVE voxels of each group, with the
+// same FP32 arithmetic as the generator warps (tc_voxel / tc_T / tc_excess) widened by kTcDelta,
+// and writes the window code the three warp roles of tc_kernel read (TcDev::codes).
+//   stats[0] = largest staged window (k-blocks), stats[1] = error bits
+//   (1: window needs more than 3 passes, 2: window leaves the zero pads, 4: negative start)
+__global__ void __launch_bounds__(kTcG * kTcRows)
+tc_window_kernel(const TcDev tp, const Params P, uint2* __restrict__ list, unsigned short* __restrict__ codes,
+                 int* __restrict__ tile_work, int* __restrict__ tile_edge, int* __restrict__ stats) {
+  __shared__ int kmn[kTcG][16], kmx[kTcG][16];
+  const int tile_i = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
+  const int g = tid / kTcRows, row = tid % kTcRows;
+  const TcTile td = tp.tiles[tile_i];
+  const TcVoxel vx = tc_voxel(tp, P, td, row, g);
+  const int Kb = (P.K + kTcBlk - 1) / kTcBlk;
+  float Tf[16];
+#pragma unroll
+  for (int q = 0; q < 16; ++q) {
+    const int qq = min(q, P.Q - 1);
+    Tf[q] = (float)(tc_T(P, vx, qq) - (double)__ldg(&tp.tbase[(long long)tile_i * P.Q + qq]));
+  }
+  const int tb4 = tid < 16 ? (__ldg(&tp.tbase[(long long)tile_i * P.Q + min(tid, P.Q - 1)]) >> 2) : 0;
+  int work = 0, edge = 0, stage = 0, err = 0;
+
+  for (int li = 0; li < td.list_cnt; ++li) {
+    const long long e = td.list_off + li;
+    if (tid < kTcG * 16) { kmn[tid / 16][tid % 16] = INT_MAX; kmx[tid / 16][tid % 16] = INT_MIN; }
+    __syncthreads();
+    const float4 el = __ldg(&P.elem[list[e].x]);
+    bool act;
+    const float ex = tc_excess(tp, P, vx, el, act);
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+      if (q < P.Q) {
+        const float t = Tf[q] + ex;
+        int lo = act ? (int)floorf(t - kTcDelta) : INT_MAX, hi = act ? (int)floorf(t + kTcDelta) : INT_MIN;
+        lo = __reduce_min_sync(0xffffffffu, lo);
+        hi = __reduce_max_sync(0xffffffffu, hi);
+        if (lane == 0 && lo != INT_MAX) { atomicMin(&kmn[g][q], lo); atomicMax(&kmx[g][q], hi); }
+      }
+    }
+    __syncthreads();
+    if (tid < 16) {
+      const int q = tid;
+      int wlo = INT_MAX, whi = INT_MIN;
+      unsigned flags = 0;
+      for (int gg = 0; gg < kTcG; ++gg) {
+        unsigned code = 0;
+        if (q < P.Q && kmn[gg][q] != INT_MAX) {
+          const int smin = kmn[gg][q], smax = kmx[gg][q];
+          if (smin < 0) err |= 4;
+          const int b0 = max(smin, 0) >> 2;
+          const int nb = ((smax + 1) >> 2) - b0 + 1;
+          const int np = (nb + kTcPassBlocks - 1) / kTcPassBlocks;
+          if (np > 3 || b0 * 2 > 0x3fff) err |= 1;
+          code = (unsigned)min(np, 3) | ((unsigned)(b0 * 2) << 2);
+          wlo = min(wlo, tb4 + b0);
+          whi = max(whi, tb4 + b0 + kTcPassBlocks * np);
+          flags |= 1u << gg;
+          work += np;
+        }
+        codes[(e * kTcG + gg) * 16 + q] = (unsigned short)code;
+      }
+      if (whi > wlo) {
+        stage = max(stage, whi - wlo);
+        if (wlo < -kTcPadBlocks || whi > Kb + kTcPadBlocks) err |= 2;
+        if (kTcBlk * wlo <= 0 || kTcBlk * whi >= P.K - 1) edge = 1;
+      }
+      flags = __reduce_or_sync(0x0000ffffu, flags);
+      if (tid == 0) list[e].y = flags;
+    }
+    __syncthreads();                                          // kmn / kmx are re-initialised at the loop top
+  }
+  if (tid < 16) {
+    work = __reduce_add_sync(0x0000ffffu, work);
+    edge = __reduce_or_sync(0x0000ffffu, edge);
+    stage = __reduce_max_sync(0x0000ffffu, stage);
+    err = __reduce_or_sync(0x0000ffffu, err);
+    if (tid == 0) {
+      tile_work[tile_i] = work;
+      tile_edge[tile_i] = edge;
+      atomicMax(&stats[0], stage);
+      if (err) atomicOr(&stats[1], err);
+    }
+  }
+}
+
 }  // namespace
+
+cudaError_t launch_tc_windows(const TcDev& tp, const Params& P, uint2* list, unsigned short* codes, int* tile_work,
+                              int* tile_edge, int* stats, cudaStream_t s) {
+  tc_window_kernel<<<tp.n_tiles, kTcG * kTcRows, 0, s>>>(tp, P, list, codes, tile_work, tile_edge, stats);
+  return cudaGetLastError();
+}
 
 cudaError_t launch_tc_kernel(const TcDev& tp, const Params& P, const void* d_conv, void* d_out, int grid, size_t smem, cudaStream_t s) {
   static bool configured = false;
@@ -299,7 +403,8 @@ cudaError_t launch_tc_kernel(const TcDev& tp, const Params& P, const void* d_con
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  tc_kernel<<<grid, kTcThreads, smem, s>>>(tp, P, static_cast<const unsigned char*>(d_conv), static_cast<float2*>(d_out));
+  static const int dbg = getenv("DAS_TC_DBG") ? atoi(getenv("DAS_TC_DBG")) : 0;
+  tc_kernel<<<grid, kTcThreads, smem, s>>>(tp, P, static_cast<const unsigned char*>(d_conv), static_cast<float2*>(d_out), dbg);
   return cudaGetLastError();
 }
 

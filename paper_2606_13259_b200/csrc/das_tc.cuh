@@ -24,14 +24,17 @@
 // frames of a chunk: the per-frame cost on the CUDA cores drops by Bc.
 //
 // Roles inside a CTA (one CTA per SM, persistent over a work-sorted tile list):
-//   warps 0..11  three generator warpgroups, one per voxel group (depth) of the tile; thread =
-//                voxel = MMA row = TMEM lane.  Per receiver: aperture test, excess path, receive
-//                phase.  Per (q, m): fractional index, weights, the 8 packed FP16 pairs of an
-//                A row -> tcgen05.st.  After the last receiver: tcgen05.ld of D -> global.
-//   warp 12      TMA producer: one bulk copy per (q, m) of the k-blocks the tile needs.
-//   warps 13..15 MMA issuers, one per voxel group (one thread each): tcgen05.mma.kind::f16,
+//   warps 0..23  generators: per voxel group (depth) of the tile two sets of 4 warps, one for the
+//                even and one for the odd transmits; thread = voxel = MMA row = TMEM lane.  Per
+//                receiver: aperture test, excess path, receive phase.  Per (q, m): fractional
+//                index, weights, the 8 packed FP16 pairs of an A row -> tcgen05.st.  After the
+//                last receiver: tcgen05.ld of D -> global (each set half of the frames).
+//   warp 24      TMA producer: one bulk copy per (q, m) of the k-blocks the tile needs.
+//   warps 25..27 MMA issuers, one per voxel group (one thread each): tcgen05.mma.kind::f16,
 //                A from TMEM, B from shared memory (K-major, no swizzle: a k-block of
 //                N columns x 16 B is one slab), D of the group in TMEM.
+//                (The issue arbiter favours high warp ids: the short, latency-critical service
+//                warps sit above the generators; the other order measured 5 % slower.)
 #pragma once
 
 #include "das_tiled.cuh"
@@ -43,15 +46,19 @@ constexpr int kTcRows = kTcGX * kTcGY;      // = 128 = MMA M
 constexpr int kTcG = 3;                     // voxel groups (consecutive depths) per tile
 constexpr int kTcBlk = 4;                   // samples per k-block (8 FP16 = 16 B per column)
 constexpr int kTcPassBlocks = 2;            // k-blocks per pass = one MMA of K = 16
-constexpr int kTcABufs = 4;                 // A ring per voxel group (TMEM), one MMA each; power of two
-constexpr int kTcStages = 4;                // shared-memory ring of staged sample windows
+constexpr int kTcMaxABufs = 8;              // A ring per voxel group (TMEM), one MMA each; depth a power of two
+constexpr int kTcMaxStages = 16;            // upper bound of the shared-memory ring of staged sample windows
+constexpr int kTcMinStages = 2;
 constexpr int kTcPadBlocks = 16;            // zero k-blocks before and after every (m, q) row
 constexpr int kTcMaxStageBlocks = 16;       // largest window (k-blocks) one stage can hold
-constexpr int kTcGenWarps = 4 * kTcG;
-constexpr int kTcThreads = (kTcGenWarps + 1 + kTcG) * 32;   // + TMA producer + one MMA issuer per group
+constexpr int kTcSets = 1;                   // generator warp sets per voxel group (2: even / odd transmits)
+constexpr int kTcQPerSet = 16 / kTcSets;
+constexpr int kTcGenWarps = 4 * kTcSets * kTcG;
+constexpr int kTcSvcWarps = 1 + kTcG;        // TMA producer + one MMA issuer per group
+constexpr int kTcThreads = (kTcSvcWarps + kTcGenWarps) * 32;
 constexpr int kTcTmemCols = 512;
 constexpr int kTcACols = 8;                 // TMEM columns of one A buffer (K = 16 FP16 per row)
-constexpr float kTcMargin = 0.02f;          // samples: slack of the plan's delay bounds
+constexpr float kTcMargin = 0.02f;          // samples: slack of the plan's transmit-delay bounds (tbase)
 
 __host__ __device__ inline int tc_kblocks(int K) { return 2 * kTcPadBlocks + (K + kTcBlk - 1) / kTcBlk; }
 
@@ -66,25 +73,88 @@ struct TcDev {
   int Bc;                      // frames per chunk; MMA N = 2 Bc
   int KBp;                     // k-blocks per (m, q) row of the converted data, pads included
   int stage_blocks;            // capacity of one stage in k-blocks
+  int n_stages;                // depth of the stage ring (kTcMinStages..kTcMaxStages)
+  int a_bufs, a_shift;         // depth of the A ring per voxel group (2^a_shift <= kTcMaxABufs, what TMEM holds)
   const TcTile* tiles;         // [n_tiles], sorted by decreasing work
-  const int2* trange;          // [n_tiles][G][Q]: floor(16 (Tmin - margin)), ceil(16 (Tmax + margin))
   const int* tbase;            // [n_tiles][Q]: sample offset of the reduced delays, multiple of 4
-  const uint4* list;           // per tile: x = m, y/z/w = group 0/1/2: elo16 | ehi16 << 16
-                               //   (bounds of 16 e over the group's active voxels); 0xFFFFFFFF = none active
+  const uint2* list;           // receiver lists of the tiles: x = m, y = bit g set if group g has a window
+  const unsigned short* codes; // [entry][G][16]: window of item (q, m) for group g, written by the plan's
+                               //   window kernel from the delays of the group's ACTIVE voxels:
+                               //   bits 0-1 = n_pass (MMAs of K = 16 = 8 samples; 0 = no active voxel),
+                               //   bits 2-15 = first sample of the window in units of 2 samples, relative
+                               //   to tbase_q
   double z_array, kappa, ratio, phase0;
   float four_f2, kappa_f, ratio_f;
 };
 
-// k-block range of group g for item (q, m); identical integer arithmetic on host and device and
-// in every warp role.  Returns the number of k-blocks (even, 0 if the group has no active voxel).
-__host__ __device__ inline int tc_block_range(int2 tr, unsigned er, int& blk_lo) {
-  if (er == 0xFFFFFFFFu) { blk_lo = 0; return 0; }
-  const int elo = (int)(er & 0xFFFFu), ehi = (int)(er >> 16);
-  const int s_lo = (tr.x + elo) >> 4;               // <= floor(t) of every active voxel
-  const int s_hi = ((tr.y + ehi) >> 4) + 1;         // >= floor(t) + 1
-  blk_lo = s_lo >> 2;
-  const int nb = (s_hi >> 2) - blk_lo + 1;
-  return (nb + 1) & ~1;
+constexpr float kTcDelta = 1.0f / 128;      // samples: the window kernel widens every delay by this much, so that
+                                            // rounding differences between it and the generator cannot matter
+__host__ __device__ inline int code_passes(unsigned c) { return (int)(c & 3u); }
+__host__ __device__ inline int code_start2(unsigned c) { return (int)(c >> 2); }   // units of 2 samples
+
+// Window of item (q, m) the producer stages: the union over the voxel groups, as (first k-block relative
+// to tbase_q / 4, number of k-blocks).  `codes_q` points at the code of group 0 for this q.
+__device__ __forceinline__ void tc_union_window(const unsigned short* codes_q, int& wlo, int& wn) {
+  int lo = 0x7fffffff, hi = -0x7fffffff;
+#pragma unroll
+  for (int g = 0; g < kTcG; ++g) {
+    const unsigned c = __ldg(&codes_q[g * 16]);
+    if (code_passes(c)) {
+      lo = min(lo, code_start2(c) >> 1);
+      hi = max(hi, (code_start2(c) >> 1) + kTcPassBlocks * code_passes(c));
+    }
+  }
+  wlo = hi > lo ? lo : 0;
+  wn = hi > lo ? hi - lo : 0;
+}
+
+// ---- geometry shared by the generator warps and the plan's window kernel ---------------------
+struct TcVoxel {
+  float x, y, z, a, a2, a2e, band;
+  double a_d;
+  int ix, iy, iz, izc;
+  bool in_grid;
+};
+// voxel of MMA row `row` (0..127: 16 x 8 lateral) in depth group g of tile td
+__device__ __forceinline__ TcVoxel tc_voxel(const TcDev& tp, const Params& P, const TcTile& td, int row, int g) {
+  TcVoxel v;
+  v.ix = td.ix0 + row % kTcGX; v.iy = td.iy0 + row / kTcGX; v.iz = td.iz0 + g;
+  v.in_grid = v.ix < P.nx && v.iy < P.ny && v.iz < P.nz;
+  v.izc = min(v.iz, P.nz - 1);
+  v.x = P.xs[min(v.ix, P.nx - 1)]; v.y = P.ys[min(v.iy, P.ny - 1)]; v.z = P.zs[v.izc];
+  v.a_d = (double)v.z - tp.z_array;
+  v.a = (float)v.a_d;
+  v.a2 = v.a * v.a;
+  v.a2e = !v.in_grid ? -1.f : (P.apod ? v.a2 : __int_as_float(0x7f800000));
+  v.band = (v.in_grid && P.apod) ? kBand * v.a2 : -1.f;
+  return v;
+}
+// the part of the sample coordinate common to all receivers: T_q(n) = (tau_tx + a / c - t_start) fs, FP64
+__device__ __forceinline__ double tc_T(const Params& P, const TcVoxel& v, int q) {
+  return (tx_delay(P.tx[q], v.x, v.y, v.z, P.c) + v.a_d / P.c - P.t_start) * P.fs;
+}
+// receive excess path e_m(n) in samples (FP32) and the exactly classified aperture weight
+__device__ __forceinline__ float tc_excess(const TcDev& tp, const Params& P, const TcVoxel& v, float4 el, bool& act) {
+  const float dx = v.x - el.x, dy = v.y - el.y;
+  const float rho2 = fmaf(dx, dx, dy * dy);
+  const float lhs = tp.four_f2 * rho2;
+  act = lhs <= v.a2e;
+  if (fabsf(lhs - v.a2e) <= v.band) act = aperture_exact(v.x, v.y, el.x, el.y, P.zs, v.izc, tp.z_array, P.fnum);
+  const float s2 = rho2 + v.a2;
+  const float d = s2 * rsqrt_approx(s2);
+  return (rho2 * tp.kappa_f) * rcp_approx(v.a + d);
+}
+
+// mbarrier wait that parks the thread in hardware (suspend-time hint, ns) instead of spinning through
+// issue slots the generator warps need; it resumes as soon as the phase completes
+__device__ __forceinline__ void mbar_wait_park(unsigned bar, unsigned parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(bar), "r"(parity), "r"(20000u) : "memory");
 }
 
 // ---- tcgen05 / TMEM PTX ----------------------------------------------------------------------
@@ -94,6 +164,12 @@ __device__ __forceinline__ void tmem_alloc(unsigned smem_dst, unsigned cols) {
 }
 __device__ __forceinline__ void tmem_dealloc(unsigned taddr, unsigned cols) {
   asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
+}
+// one lane of the (converged) warp
+__device__ __forceinline__ bool tc_elect() {
+  unsigned pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -138,15 +214,15 @@ __device__ __forceinline__ unsigned pack_half2(float lo, float hi) {
 }
 
 struct alignas(128) TcSmemHeader {
-  unsigned long long b_full[kTcStages], b_empty[kTcStages];
-  unsigned long long a_full[kTcG][kTcABufs], a_empty[kTcG][kTcABufs];
+  unsigned long long b_full[kTcMaxStages], b_empty[kTcMaxStages];
+  unsigned long long a_full[kTcG * kTcMaxABufs], a_empty[kTcG * kTcMaxABufs];
   unsigned long long d_full, d_empty;
-  int wlo[kTcStages];                // first k-block of the staged window (producer -> MMA issuer)
+  unsigned long long sink;           // arrivals nobody waits for (no A tile in flight)
   unsigned tmem_base;
 };
 
-__host__ __device__ inline size_t tc_smem_bytes(int Bc, int stage_blocks) {
-  return sizeof(TcSmemHeader) + 128 + (size_t)kTcStages * stage_blocks * (2 * Bc) * 16;
+__host__ __device__ inline size_t tc_smem_bytes(int Bc, int stage_blocks, int n_stages) {
+  return sizeof(TcSmemHeader) + 128 + (size_t)n_stages * stage_blocks * (2 * Bc) * 16;
 }
 
 struct TcPlan;
@@ -155,6 +231,8 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& desc, int n_frame
 void tc_plan_destroy(TcPlan* tp);
 size_t tc_converted_bytes(const TcPlan* tp, const Params& P);
 int tc_frames_per_chunk(const TcPlan* tp);
+cudaError_t launch_tc_windows(const TcDev& tp, const Params& P, uint2* list, unsigned short* codes, int* tile_work,
+                              int* tile_edge, int* stats, cudaStream_t s);
 cudaError_t launch_tc(const TcPlan* tp, const Params& P, const void* d_conv, void* d_out, cudaStream_t s);
 cudaError_t launch_convert_batch(const TcPlan* tp, const Params& P, const void* d_raw, void* d_conv,
                                  float scale, cudaStream_t s);

@@ -3,6 +3,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <numeric>
 #include <vector>
@@ -43,7 +44,6 @@ cudaError_t up(TcPlan* tp, const std::vector<T>& h, const T** d_out) {
   *d_out = static_cast<const T*>(d);
   return e;
 }
-inline double excess(double rho, double a) { return rho * rho / (a + std::sqrt(rho * rho + a * a)); }
 }  // namespace
 
 TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, int device, char* why,
@@ -74,15 +74,12 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
   const long long n_tiles_ll = (long long)ntx * nty * ntz;
   if (n_tiles_ll > (1 << 22)) return refuse("too many tiles");
   const int n_tiles = (int)n_tiles_ll;
-  const int Kb = (P.K + kTcBlk - 1) / kTcBlk;
 
+  // ---- host part: tiles, sample base per (tile, q), conservative receiver lists ------------------
   std::vector<TcTile> tiles(n_tiles);
-  std::vector<int2> trange((size_t)n_tiles * kTcG * Q);
   std::vector<int> tbase((size_t)n_tiles * Q);
-  std::vector<uint4> list;
-  std::vector<double> work(n_tiles, 0.0);
+  std::vector<uint2> list;
   list.reserve((size_t)n_tiles * std::min(M, 512));
-  int stage_blocks = 2;
   const double cone = apod ? 1.0 / (2.0 * fnum) : 0.0;
 
   int t = 0;
@@ -93,75 +90,97 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
         td.ix0 = txi * kTcGX; td.iy0 = ty * kTcGY; td.iz0 = tz * kTcG;
         td.edge = 0;
         const int ix1 = std::min(td.ix0 + kTcGX, d.nx), iy1 = std::min(td.iy0 + kTcGY, d.ny);
+        const int iz1 = std::min(td.iz0 + kTcG, d.nz);
         double xlo = 1e300, xhi = -1e300, ylo = 1e300, yhi = -1e300;
         for (int i = td.ix0; i < ix1; ++i) { xlo = std::min(xlo, (double)d.xs[i]); xhi = std::max(xhi, (double)d.xs[i]); }
         for (int i = td.iy0; i < iy1; ++i) { ylo = std::min(ylo, (double)d.ys[i]); yhi = std::max(yhi, (double)d.ys[i]); }
-        // ---- transmit part: exact min / max of T_q over the voxels of each group ------------
-        int tlo_tile[16];
-        for (int q = 0; q < Q; ++q) tlo_tile[q] = 0x7fffffff;
-        for (int g = 0; g < kTcG; ++g) {
-          const int iz = std::min(td.iz0 + g, d.nz - 1);
-          const double z = d.zs[iz], a = z - z_a;
-          for (int q = 0; q < Q; ++q) {
-            const das_transmit_t& tx = d.tx[q];
-            double lo = 1e300, hi = -1e300;
+        // sample base: a multiple of 4 below T_q of every voxel of the tile (the kernels clamp the rows
+        // and columns beyond the grid edge to the last voxel, which is inside these ranges)
+        for (int q = 0; q < Q; ++q) {
+          const das_transmit_t& tx = d.tx[q];
+          double lo = 1e300;
+          for (int k = td.iz0; k < iz1; ++k) {
+            const double z = d.zs[k], a = z - z_a;
             for (int i = td.ix0; i < ix1; ++i)
               for (int j = td.iy0; j < iy1; ++j) {
                 const double x = d.xs[i], y = d.ys[j];
                 double tau;
                 if (tx.type == DAS_TX_PLANE) tau = (x * tx.v[0] + y * tx.v[1] + z * tx.v[2]) / c + tx.t0;
                 else tau = std::sqrt((x - tx.v[0]) * (x - tx.v[0]) + (y - tx.v[1]) * (y - tx.v[1]) + (z - tx.v[2]) * (z - tx.v[2])) / c + tx.t0;
-                const double T = (tau + a / c - t_start) * fs;
-                lo = std::min(lo, T); hi = std::max(hi, T);
+                lo = std::min(lo, (tau + a / c - t_start) * fs);
               }
-            if (!(std::fabs(lo) < 1e8 && std::fabs(hi) < 1e8)) return refuse("sample coordinate out of range");
-            const int l16 = (int)std::floor(16.0 * (lo - kTcMargin)), h16 = (int)std::ceil(16.0 * (hi + kTcMargin));
-            trange[((size_t)t * kTcG + g) * Q + q] = make_int2(l16, h16);
-            tlo_tile[q] = std::min(tlo_tile[q], l16);
           }
+          if (!(std::fabs(lo) < 1e8)) return refuse("sample coordinate out of range");
+          tbase[(size_t)t * Q + q] = (int)std::floor((lo - kTcMargin) / 4.0) * 4;
         }
-        for (int q = 0; q < Q; ++q) tbase[(size_t)t * Q + q] = ((tlo_tile[q] >> 4) >> 2) * 4;   // multiple of 4, <= every floor(T)
-        // ---- receiver part: list of receivers seen by any group, bounds of e per group --------
+        // receivers whose aperture cone can reach a voxel of the tile (bounding-box test; the window
+        // kernel below classifies every voxel exactly and drops the receivers no group sees)
         td.list_off = (int)list.size();
+        const double a_max = (double)d.zs[iz1 - 1] - z_a, a_min = (double)d.zs[td.iz0] - z_a;
+        const double a_far = std::max(a_max, a_min);
         for (int m = 0; m < M; ++m) {
           const double ex = d.elem_pos[3 * m], ey = d.elem_pos[3 * m + 1];
           const double nx_ = std::max(std::max(xlo - ex, ex - xhi), 0.0), ny_ = std::max(std::max(ylo - ey, ey - yhi), 0.0);
-          const double fx = std::max(std::fabs(xlo - ex), std::fabs(xhi - ex)), fy = std::max(std::fabs(ylo - ey), std::fabs(yhi - ey));
-          const double rho_min = std::sqrt(nx_ * nx_ + ny_ * ny_), rho_max = std::sqrt(fx * fx + fy * fy);
-          unsigned er[kTcG];
-          bool any = false;
-          for (int g = 0; g < kTcG; ++g) {
-            er[g] = 0xFFFFFFFFu;
-            if (td.iz0 + g >= d.nz) continue;
-            const double a = (double)d.zs[td.iz0 + g] - z_a;
-            if (apod && rho_min > cone * a * (1.0 + 1e-5)) continue;                 // no voxel of the group sees m
-            const double r_hi = apod ? std::min(rho_max, cone * a * (1.0 + 1e-5)) : rho_max;
-            const double e_lo = excess(rho_min, a) * kappa - kTcMargin, e_hi = excess(r_hi, a) * kappa + kTcMargin;
-            const int l16 = std::max((int)std::floor(16.0 * e_lo), 0), h16 = (int)std::ceil(16.0 * e_hi);
-            if (h16 > 0xFFFE) return refuse("receive delay exceeds the 16-bit bound format");
-            er[g] = (unsigned)l16 | ((unsigned)h16 << 16);
-            any = true;
-          }
-          if (!any) continue;
-          list.push_back(make_uint4((unsigned)m, er[0], er[1], er[2]));
-          // stage size and row bounds for every transmit
-          for (int q = 0; q < Q; ++q) {
-            int wlo = 0x7fffffff, whi = -0x7fffffff;
-            for (int g = 0; g < kTcG; ++g) {
-              int lo;
-              const int nb = tc_block_range(trange[((size_t)t * kTcG + g) * Q + q], er[g], lo);
-              if (nb) { wlo = std::min(wlo, lo); whi = std::max(whi, lo + nb); work[t] += nb; }
-            }
-            if (whi > wlo) {
-              stage_blocks = std::max(stage_blocks, whi - wlo);
-              if (wlo < -kTcPadBlocks || whi > Kb + kTcPadBlocks) return refuse("a sample window leaves the zero-padded record");
-              if (kTcBlk * wlo <= 0 || kTcBlk * whi >= P.K - 1) td.edge = 1;
-            }
-          }
+          const double rho_min = std::sqrt(nx_ * nx_ + ny_ * ny_);
+          if (apod && rho_min > cone * a_far * (1.0 + 1e-5)) continue;
+          list.push_back(make_uint2((unsigned)m, 0u));
         }
         td.list_cnt = (int)list.size() - td.list_off;
       }
-  if (stage_blocks > kTcMaxStageBlocks) { snprintf(why, why_len, "sample window per tile (%d k-blocks) exceeds the stage capacity (%d)", stage_blocks, kTcMaxStageBlocks); return nullptr; }
+  if (list.size() > (size_t)0x7fffffff / (kTcG * 16)) return refuse("receiver lists too long");
+
+  TcPlan* tp = new TcPlan();
+  tp->n_frames = n_frames;
+  cudaDeviceProp prop;
+  cudaError_t e = cudaGetDeviceProperties(&prop, device);
+  if (e != cudaSuccess) { *cuda_err = e; delete tp; return nullptr; }
+  TcDev& dv = tp->dev;
+  dv.n_tiles = n_tiles;
+  dv.Bc = Bc;
+  dv.n_chunks = n_frames / Bc;
+  dv.KBp = tc_kblocks(P.K);
+  dv.z_array = z_a; dv.kappa = kappa; dv.ratio = fc / fs;
+  dv.phase0 = fc * t_start - std::floor(fc * t_start);
+  dv.four_f2 = (float)(4.0 * fnum * fnum);
+  dv.kappa_f = (float)kappa; dv.ratio_f = (float)(fc / fs);
+
+  // ---- device part: exact windows per (receiver, transmit, voxel group) ---------------------------
+  auto fail = [&](cudaError_t ce) -> TcPlan* { *cuda_err = ce; tc_plan_destroy(tp); return nullptr; };
+  const TcTile* d_tiles0 = nullptr;
+  const int* d_tbase0 = nullptr;
+  void *d_codes = nullptr, *d_work = nullptr, *d_edge = nullptr, *d_stats = nullptr;
+  if ((e = up(tp, tiles, &d_tiles0)) != cudaSuccess || (e = up(tp, tbase, &d_tbase0)) != cudaSuccess ||
+      (e = up(tp, list, &dv.list)) != cudaSuccess) return fail(e);
+  const size_t n_codes = std::max<size_t>(list.size(), 1) * kTcG * 16;
+  if ((e = cudaMalloc(&d_codes, n_codes * sizeof(unsigned short))) != cudaSuccess) return fail(e);
+  tp->allocs.push_back(d_codes);
+  if ((e = cudaMalloc(&d_work, sizeof(int) * n_tiles)) != cudaSuccess) return fail(e);
+  tp->allocs.push_back(d_work);
+  if ((e = cudaMalloc(&d_edge, sizeof(int) * n_tiles)) != cudaSuccess) return fail(e);
+  tp->allocs.push_back(d_edge);
+  if ((e = cudaMalloc(&d_stats, sizeof(int) * 2)) != cudaSuccess) return fail(e);
+  tp->allocs.push_back(d_stats);
+  if ((e = cudaMemset(d_stats, 0, sizeof(int) * 2)) != cudaSuccess) return fail(e);
+  dv.tiles = d_tiles0;
+  dv.tbase = d_tbase0;
+  dv.codes = static_cast<const unsigned short*>(d_codes);
+  if ((e = launch_tc_windows(dv, P, const_cast<uint2*>(dv.list), static_cast<unsigned short*>(d_codes), static_cast<int*>(d_work),
+                             static_cast<int*>(d_edge), static_cast<int*>(d_stats), nullptr)) != cudaSuccess) return fail(e);
+  std::vector<int> work(n_tiles), edge(n_tiles);
+  int stats[2] = {0, 0};
+  if ((e = cudaMemcpy(work.data(), d_work, sizeof(int) * n_tiles, cudaMemcpyDeviceToHost)) != cudaSuccess ||
+      (e = cudaMemcpy(edge.data(), d_edge, sizeof(int) * n_tiles, cudaMemcpyDeviceToHost)) != cudaSuccess ||
+      (e = cudaMemcpy(stats, d_stats, sizeof(stats), cudaMemcpyDeviceToHost)) != cudaSuccess) return fail(e);
+  auto refuse_free = [&](const char* msg) -> TcPlan* { tc_plan_destroy(tp); return refuse(msg); };
+  if (stats[1] & 1) return refuse_free("a sample window of a voxel group needs more than 3 MMA passes (grid too coarse)");
+  if (stats[1] & 2) return refuse_free("a sample window leaves the zero-padded record");
+  if (stats[1] & 4) return refuse_free("internal: negative window start");
+  const int stage_blocks = std::max(stats[0], kTcPassBlocks);
+  if (stage_blocks > kTcMaxStageBlocks) {
+    snprintf(why, why_len, "sample window per tile (%d k-blocks) exceeds the stage capacity (%d)", stage_blocks, kTcMaxStageBlocks);
+    tc_plan_destroy(tp);
+    return nullptr;
+  }
 
   // Tile order: depth slab by depth slab (heaviest slab first), all lateral tiles of a slab side by
   // side.  The CTAs of a wave then walk the same receivers of the same depth at about the same
@@ -177,36 +196,28 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
     return work[a] > work[b];
   });
   std::vector<TcTile> tiles_s(n_tiles);
-  std::vector<int2> trange_s(trange.size());
   std::vector<int> tbase_s(tbase.size());
   for (int i = 0; i < n_tiles; ++i) {
     tiles_s[i] = tiles[order[i]];
-    std::memcpy(&trange_s[(size_t)i * kTcG * Q], &trange[(size_t)order[i] * kTcG * Q], sizeof(int2) * kTcG * Q);
+    tiles_s[i].edge = edge[order[i]];
     std::memcpy(&tbase_s[(size_t)i * Q], &tbase[(size_t)order[i] * Q], sizeof(int) * Q);
   }
+  if ((e = up(tp, tiles_s, &dv.tiles)) != cudaSuccess || (e = up(tp, tbase_s, &dv.tbase)) != cudaSuccess) return fail(e);
 
-  TcPlan* tp = new TcPlan();
-  tp->n_frames = n_frames;
-  cudaDeviceProp prop;
-  cudaError_t e = cudaGetDeviceProperties(&prop, device);
-  if (e != cudaSuccess) { *cuda_err = e; delete tp; return nullptr; }
-  TcDev& dv = tp->dev;
-  dv.n_tiles = n_tiles;
-  dv.Bc = Bc;
-  dv.n_chunks = n_frames / Bc;
-  dv.KBp = tc_kblocks(P.K);
   dv.stage_blocks = stage_blocks;
-  dv.z_array = z_a; dv.kappa = kappa; dv.ratio = fc / fs;
-  dv.phase0 = fc * t_start - std::floor(fc * t_start);
-  dv.four_f2 = (float)(4.0 * fnum * fnum);
-  dv.kappa_f = (float)kappa; dv.ratio_f = (float)(fc / fs);
-  tp->smem = tc_smem_bytes(Bc, stage_blocks);
-  if (tp->smem > 200 * 1024) { delete tp; return refuse("stage ring does not fit in shared memory"); }
+  // A ring: as deep as tensor memory allows next to the accumulators (512 columns: kTcG * 2 Bc of D)
+  dv.a_shift = 3;
+  if (const char* ev = getenv("DAS_TC_ABUFS")) dv.a_shift = std::min(3, std::max(0, atoi(ev)));   // tuning sweeps only
+  while (dv.a_shift > 0 && kTcG * 2 * Bc + kTcG * (1 << dv.a_shift) * kTcACols > kTcTmemCols) --dv.a_shift;
+  dv.a_bufs = 1 << dv.a_shift;
+  // The ring only has to cover the L2 latency of a window: measured flat from 4 to 8 stages at the
+  // headline, slower at 16 (the CTAs drift apart and L2 holds fewer of their shared windows).
+  dv.n_stages = 6;
+  if (const char* ev = getenv("DAS_TC_STAGES")) dv.n_stages = std::min(kTcMaxStages, std::max(kTcMinStages, atoi(ev)));   // tuning sweeps only
+  while (dv.n_stages > kTcMinStages && tc_smem_bytes(Bc, stage_blocks, dv.n_stages) > 200 * 1024) --dv.n_stages;
+  tp->smem = tc_smem_bytes(Bc, stage_blocks, dv.n_stages);
+  if (tp->smem > 200 * 1024) return refuse_free("stage ring does not fit in shared memory");
   tp->grid = std::max(1, std::min(n_tiles * dv.n_chunks, prop.multiProcessorCount));
-  if ((e = up(tp, tiles_s, &dv.tiles)) != cudaSuccess || (e = up(tp, trange_s, &dv.trange)) != cudaSuccess ||
-      (e = up(tp, tbase_s, &dv.tbase)) != cudaSuccess || (e = up(tp, list, &dv.list)) != cudaSuccess) {
-    *cuda_err = e; tc_plan_destroy(tp); return nullptr;
-  }
   return tp;
 }
 
