@@ -8,15 +8,9 @@ namespace das {
 
 namespace {
 
-// (first k-block, passes) of one (q, m) item for one voxel group, packed so that one shuffle hands
-// it from the lane that worked it out (lane = q) to the whole warp
-__device__ __forceinline__ int pack_item(int blk, int n_pass) { return (blk << 2) | n_pass; }
-__device__ __forceinline__ int item_passes(int pk) { return pk & 3; }
-__device__ __forceinline__ int item_blk(int pk) { return pk >> 2; }
-
 // Work items: (chunk, tile), tile fastest; every warp role walks the same sequence.
 __global__ void __launch_bounds__(kTcThreads, 1)
-tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ convb, float2* __restrict__ out, const int dbg) {
+tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ convb, float2* __restrict__ out) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   TcSmemHeader& sm = *reinterpret_cast<TcSmemHeader*>(smem_raw);
   const unsigned stage0 = (smem_u32(smem_raw) + (unsigned)sizeof(TcSmemHeader) + 127u) & ~127u;
@@ -36,7 +30,7 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
   if (tid == 0) {
     for (int s = 0; s < kTcMaxStages; ++s) { mbar_init(b_full0 + 8 * s, 1); mbar_init(b_empty0 + 8 * s, kTcG); }
     for (int i = 0; i < kTcMaxABufs * kTcG; ++i) { mbar_init(a_full0 + 8 * i, 4); mbar_init(a_empty0 + 8 * i, 1); }
-    mbar_init(d_full, kTcG);
+    mbar_init(d_full, kTcG * kTcIssuers);
     mbar_init(d_empty, kTcGenWarps);
     mbar_init(smem_u32(&sm.sink), 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -49,6 +43,16 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
   // TMEM columns: D of group g at g * N; A buffer (g, buf) at kTcG * N + (a_bufs g + buf) * kTcACols
   const unsigned a_col0 = (unsigned)(kTcG * N);
   const unsigned nab = (unsigned)tp.a_bufs, nab_sh = (unsigned)tp.a_shift;   // A ring depth (power of two)
+  // The accumulators start from zero and the epilogue leaves them zero again, so every MMA accumulates
+  // and no MMA has to be the first (kTcIssuers warps of a group need no order between them).
+  if (warp < kTcGenWarps) {
+    const unsigned d0 = tmem + (((unsigned)((warp & 3) * 32)) << 16) + (unsigned)((warp >> 2) * N);
+    for (int c0 = 0; c0 < N; c0 += 8) tmem_st8_zero(d0 + (unsigned)c0);
+    tmem_wait_st();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
 
   if (warp == kTcGenWarps) {
     // ===================================== TMA PRODUCER =======================================
@@ -87,11 +91,12 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
     }
   } else if (warp > kTcGenWarps) {
     // ===================================== MMA ISSUERS ========================================
-    // One warp per voxel group.  The issue loop is a serial chain (wait -> MMA -> commit), so it is
+    // kTcIssuers warps per voxel group share the items (q, m) by the parity of q.  The issue loop is
+    // a serial chain (wait -> MMA -> commit) whose latency bounds the MMA rate of a group, so it is
     // kept as short as it can be: lane q prepares item (q, m) (passes, offset of the group's window
     // inside the staged one), every lane runs the same scalar loop (no divergence, one shuffle per
     // item), and only the tcgen05 instructions sit under an elected lane.
-    const int g = warp - kTcGenWarps - 1;
+    const int g = (warp - kTcGenWarps - 1) / kTcIssuers, par = (warp - kTcGenWarps - 1) % kTcIssuers;
     const unsigned idesc = tc_idesc(N);
     const unsigned d_tmem = tmem + (unsigned)(g * N);
     const unsigned a_tmem0 = tmem + a_col0 + (nab * (unsigned)g) * kTcACols;
@@ -104,7 +109,6 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
       const TcTile td = tp.tiles[tile_i];
       mbar_wait_park(d_empty, (n_done & 1u) ^ 1u);             // epilogue of the previous tile has drained D
       tc_fence_after();
-      unsigned acc = 0;
       for (int li = 0; li < td.list_cnt; ++li) {
         const long long e = td.list_off + li;
         const uint2 hd = __ldg(&tp.list[e]);
@@ -118,6 +122,9 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
         for (int q = 0; q < P.Q; ++q) {
           const unsigned info = __shfl_sync(0xffffffffu, info_l, q);
           const int np = (int)(info & 3u);
+          if ((q % kTcIssuers) != par) {                      // the other warp's item: count its ring slots
+            a_it += (unsigned)np;
+          } else {
           mbar_wait_park(b_full0 + 8 * s, ph);                 // also keeps an idle group in step with the ring
           if (np) {
             unsigned long long desc = desc0 + (unsigned long long)(((stage0 + s * stage_bytes) >> 4) + (info >> 2));
@@ -126,14 +133,14 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
               mbar_wait_park(af0 + 8u * buf, (a_it >> nab_sh) & 1u);
               tc_fence_after();
               if (tc_elect()) {
-                if (!(dbg & 1)) tc_mma_ts(d_tmem, a_tmem0 + buf * kTcACols, desc, idesc, acc);
+                tc_mma_ts(d_tmem, a_tmem0 + buf * kTcACols, desc, idesc, 1u);
                 tc_commit(ae0 + 8u * buf);                     // A buffer free once this MMA has read it
               }
-              acc = 1;
             }
             if (tc_elect()) tc_commit(b_empty0 + 8 * s);       // this group is done with the stage
           } else if (lane == 0) {
             mbar_arrive(b_empty0 + 8 * s);                     // nothing to read: release at once
+          }
           }
           if (++s == (unsigned)tp.n_stages) { s = 0; ph ^= 1u; }
         }
@@ -142,10 +149,7 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
     }
   } else {
     // ===================================== GENERATORS =========================================
-    // Two warp sets per voxel group share the transmits (set h takes q = 2 j + h): twice the warps
-    // to hide the latencies of the per-pass chain (shuffle -> index -> weights -> placement -> store).
-    const int g = warp / (4 * kTcSets);                       // voxel group = depth inside the tile
-    const int h = (warp >> 2) % kTcSets;                      // this warp set takes the transmits q = kTcSets j + h
+    const int g = warp >> 2;                                  // voxel group = depth inside the tile
     const int row = (warp & 3) * 32 + lane;                   // MMA row = TMEM lane (quarter warp % 4)
     const unsigned lane_base = ((unsigned)((warp & 3) * 32)) << 16;
     const unsigned d_addr = tmem + lane_base + (unsigned)(g * N);
@@ -153,9 +157,6 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
     const unsigned af0 = a_full0 + 8u * (nab * (unsigned)g), ae0 = a_empty0 + 8u * (nab * (unsigned)g);
     const bool lane0 = lane == 0;
     const bool lane_has_q = (lane & 15) < P.Q;
-    // epilogue columns of this set: half of D each when a half is a whole number of 16-column loads
-    const bool split = kTcSets == 2 && (N % 32) == 0;
-    const int col_lo = split ? h * (N / 2) : 0, col_hi = split ? col_lo + N / 2 : (h == 0 ? N : 0);
     unsigned a_it = 0, n_done = 0;
     // a_full barrier of the A tile whose store is in flight; a sink nobody waits on while there is none
     unsigned pend = smem_u32(&sm.sink);
@@ -166,11 +167,11 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
       const TcVoxel vx = tc_voxel(tp, P, td, row, g);
       const int tb_l = __ldg(&tp.tbase[(long long)tile_i * P.Q + ql]);
 
-      // per-(q, n) part in FP64: reduced transmit delay and transmit phase factor, q = 2 j + h
-      float Tf[kTcQPerSet], pc[kTcQPerSet], ps[kTcQPerSet];
+      // per-(q, n) part in FP64: reduced transmit delay and transmit phase factor
+      float Tf[16], pc[16], ps[16];
 #pragma unroll
-      for (int j = 0; j < kTcQPerSet; ++j) {
-        const int qq = min(kTcSets * j + h, P.Q - 1);
+      for (int j = 0; j < 16; ++j) {
+        const int qq = min(j, P.Q - 1);
         const double T = tc_T(P, vx, qq);
         Tf[j] = (float)(T - (double)__ldg(&tp.tbase[(long long)tile_i * P.Q + qq]));
         double cyc = tp.phase0 + tp.ratio * T;
@@ -179,7 +180,6 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
         pc[j] = cos_approx(ang);
         ps[j] = sin_approx(ang);
       }
-      bool produced = false;
 
       // the list entry one iteration ahead: header, this lane's window code, receiver position
       uint2 hd_n = make_uint2(0u, 0u);
@@ -208,20 +208,10 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
         cyc -= rintf(cyc);
         const float ang = 6.283185307179586f * cyc;
         const float pr = act ? cos_approx(ang) : 0.f, pi = act ? sin_approx(ang) : 0.f;
-        produced = true;
 
 #pragma unroll
-        for (int j = 0; j < kTcQPerSet; ++j) {
-          // items in transmit order; with two warp sets q = 2 j belongs to set 0 and q = 2 j + 1 to
-          // set 1, and the ring slots of the other set's item are counted, not written
-          unsigned c_q, c_e = 0u, c_o = 0u;
-          if (kTcSets == 2) {
-            c_e = __shfl_sync(0xffffffffu, cl, 2 * j); c_o = __shfl_sync(0xffffffffu, cl, 2 * j + 1);
-            c_q = h ? c_o : c_e;
-            a_it += h ? (unsigned)code_passes(c_e) : 0u;
-          } else {
-            c_q = __shfl_sync(0xffffffffu, cl, j);
-          }
+        for (int j = 0; j < 16; ++j) {                           // items in transmit order, q = j
+          const unsigned c_q = __shfl_sync(0xffffffffu, cl, j);
           const int n_pass = code_passes(c_q);
           // fractional index: ki = floor(t) (round-to-nearest of t - 1/2), al = t - ki
           const float t = Tf[j] + ex;
@@ -237,7 +227,7 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
           if (td.edge) {
             // reading A6: the term is dropped unless 0 <= k <= K-2 (a pad sample may not lend its
             // neighbour a weight); only tiles whose windows touch the ends of the record get here
-            const int tb_q = __shfl_sync(0xffffffffu, tb_l, min(kTcSets * j + h, P.Q - 1));
+            const int tb_q = __shfl_sync(0xffffffffu, tb_l, min(j, P.Q - 1));
             const int ki = (int)(__float_as_uint(u) - kMagicBits);
             if ((unsigned)(ki + tb_q) > (unsigned)(P.K - 2)) { w0 = 0u; w1 = 0u; }
           }
@@ -247,7 +237,6 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
             unsigned v[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) v[i] = 0u;
-            if (!(dbg & 2))
 #pragma unroll
             for (int i = -1; i < 8; ++i) {
               const bool hit = r == i;
@@ -256,16 +245,15 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
             }
             const unsigned buf = a_it & (nab - 1u);
             // complete the previous A tile (its store has had the placement above to land)
-            if (!(dbg & 8)) tmem_wait_st();
+            tmem_wait_st();
             tc_fence_before();
             if (lane0) mbar_arrive(pend);
-            if (!(dbg & 32)) mbar_wait_park(ae0 + 8u * buf, ((a_it >> nab_sh) & 1u) ^ 1u);
+            mbar_wait_park(ae0 + 8u * buf, ((a_it >> nab_sh) & 1u) ^ 1u);
             tc_fence_after();
-            if (!(dbg & 16)) tmem_st8(a_addr0 + buf * kTcACols, v);
+            tmem_st8(a_addr0 + buf * kTcACols, v);
             pend = af0 + 8u * buf;
             ++a_it;
           }
-          if (kTcSets == 2) a_it += h ? 0u : (unsigned)code_passes(c_o);
         }
       }
       tmem_wait_st();
@@ -278,16 +266,19 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
       tc_fence_after();
       const long long vox = ((long long)vx.ix * P.ny + vx.iy) * P.nz + vx.iz;
       float2* dst = out + (long long)chunk * tp.Bc * n_vox + vox;
-      for (int c0 = col_lo; c0 < col_hi; c0 += 16) {
+      for (int c0 = 0; c0 < N; c0 += 16) {
         float v[16];
         tmem_ld16(d_addr + (unsigned)c0, v);
         tmem_wait_ld();
         if (vx.in_grid) {
 #pragma unroll
           for (int i = 0; i < 8; ++i)
-            dst[(long long)(c0 / 2 + i) * n_vox] = produced ? make_float2(v[2 * i], v[2 * i + 1]) : make_float2(0.f, 0.f);
+            dst[(long long)(c0 / 2 + i) * n_vox] = make_float2(v[2 * i], v[2 * i + 1]);
         }
+        tmem_st8_zero(d_addr + (unsigned)c0);                  // leave the accumulator zero for the next tile
+        tmem_st8_zero(d_addr + (unsigned)c0 + 8u);
       }
+      tmem_wait_st();
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(d_empty);
@@ -403,8 +394,7 @@ cudaError_t launch_tc_kernel(const TcDev& tp, const Params& P, const void* d_con
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  static const int dbg = getenv("DAS_TC_DBG") ? atoi(getenv("DAS_TC_DBG")) : 0;
-  tc_kernel<<<grid, kTcThreads, smem, s>>>(tp, P, static_cast<const unsigned char*>(d_conv), static_cast<float2*>(d_out), dbg);
+  tc_kernel<<<grid, kTcThreads, smem, s>>>(tp, P, static_cast<const unsigned char*>(d_conv), static_cast<float2*>(d_out));
   return cudaGetLastError();
 }
 

@@ -24,17 +24,17 @@
 // frames of a chunk: the per-frame cost on the CUDA cores drops by Bc.
 //
 // Roles inside a CTA (one CTA per SM, persistent over a work-sorted tile list):
-//   warps 0..23  generators: per voxel group (depth) of the tile two sets of 4 warps, one for the
-//                even and one for the odd transmits; thread = voxel = MMA row = TMEM lane.  Per
-//                receiver: aperture test, excess path, receive phase.  Per (q, m): fractional
-//                index, weights, the 8 packed FP16 pairs of an A row -> tcgen05.st.  After the
-//                last receiver: tcgen05.ld of D -> global (each set half of the frames).
-//   warp 24      TMA producer: one bulk copy per (q, m) of the k-blocks the tile needs.
-//   warps 25..27 MMA issuers, one per voxel group (one thread each): tcgen05.mma.kind::f16,
-//                A from TMEM, B from shared memory (K-major, no swizzle: a k-block of
-//                N columns x 16 B is one slab), D of the group in TMEM.
-//                (The issue arbiter favours high warp ids: the short, latency-critical service
-//                warps sit above the generators; the other order measured 5 % slower.)
+//   warps 0..11  generators, 4 warps per voxel group (depth) of the tile; thread = voxel = MMA row
+//                = TMEM lane.  Per receiver: aperture test, excess path, receive phase.  Per
+//                (q, m): fractional index, weights, the 8 packed FP16 pairs of an A row ->
+//                tcgen05.st.  After the last receiver: tcgen05.ld of D -> global, D zeroed again.
+//   warp 12      TMA producer: one bulk copy per (q, m) of the k-blocks the tile needs.
+//   warps 13..15 MMA issuers, one per voxel group: tcgen05.mma.kind::f16, A from TMEM, B from
+//                shared memory (K-major, no swizzle: a k-block of N columns x 16 B is one slab),
+//                D of the group in TMEM.  The issue loop is a serial latency chain (wait, MMA,
+//                commit): every lane runs it, only the tcgen05 instructions sit under elect.sync.
+//   (The issue arbiter favours high warp ids: the short, latency-critical service warps sit above
+//   the generators; the other order measured 5 % slower.)
 #pragma once
 
 #include "das_tiled.cuh"
@@ -51,10 +51,11 @@ constexpr int kTcMaxStages = 16;            // upper bound of the shared-memory 
 constexpr int kTcMinStages = 2;
 constexpr int kTcPadBlocks = 16;            // zero k-blocks before and after every (m, q) row
 constexpr int kTcMaxStageBlocks = 16;       // largest window (k-blocks) one stage can hold
-constexpr int kTcSets = 1;                   // generator warp sets per voxel group (2: even / odd transmits)
-constexpr int kTcQPerSet = 16 / kTcSets;
-constexpr int kTcGenWarps = 4 * kTcSets * kTcG;
-constexpr int kTcSvcWarps = 1 + kTcG;        // TMA producer + one MMA issuer per group
+constexpr int kTcGenWarps = 4 * kTcG;
+constexpr int kTcIssuers = 1;                // MMA issuer warps per voxel group (2 share the items by the parity of q:
+                                             // correct, but measured 152 ms against 130 ms per 64-frame batch at the
+                                             // headline: the extra warps take issue slots from the generators)
+constexpr int kTcSvcWarps = 1 + kTcIssuers * kTcG;   // TMA producer + the MMA issuers
 constexpr int kTcThreads = (kTcSvcWarps + kTcGenWarps) * 32;
 constexpr int kTcTmemCols = 512;
 constexpr int kTcACols = 8;                 // TMEM columns of one A buffer (K = 16 FP16 per row)
@@ -187,6 +188,9 @@ __device__ __forceinline__ void tc_mma_ts(unsigned d_tmem, unsigned a_tmem, unsi
 __device__ __forceinline__ void tmem_st8(unsigned taddr, const unsigned (&v)[8]) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
                ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]) : "memory");
+}
+__device__ __forceinline__ void tmem_st8_zero(unsigned taddr) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1};" ::"r"(taddr), "r"(0u) : "memory");
 }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
