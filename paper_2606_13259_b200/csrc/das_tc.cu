@@ -8,6 +8,84 @@ namespace das {
 
 namespace {
 
+// Ring state of one generator warp: the A tiles of its voxel group in tensor memory.
+struct TcGenRing {
+  unsigned a_it;        // passes written so far (slot = a_it mod depth, phase = a_it / depth)
+  unsigned pend;        // a_full barrier of the A tile whose store is in flight (a sink while there is none)
+  unsigned nab, nab_sh; // ring depth and its log2
+  unsigned ae0, af0;    // first a_empty / a_full barrier of the group
+  unsigned a_addr0;     // TMEM address of slot 0 for this warp's lane quarter
+  bool lane0;
+};
+
+// One (q, m) item of a generator thread: the two packed weights, the slot of sample k, the passes.
+struct TcItem { unsigned w0, w1; int r, n_pass; };
+
+// All 16 items of one receiver for one voxel row.  cw[] holds the 16 window codes of the group
+// (two per word, loaded with one address for the whole warp: no shuffle in the chain).  The item
+// math of q + 1 is written before the stores of q, so that it fills the latency of the
+// store / barrier sequence.  EDGE: the tile's windows touch the ends of the record (reading A6).
+template <bool EDGE>
+__device__ __forceinline__ void tc_gen_receiver(const float (&Tf)[16], const float (&pc)[16], const float (&ps)[16],
+                                                const float ex, const float pr, const float pi, const uint4 cw0,
+                                                const uint4 cw1, const int tb_l, const int Q, const int K, TcGenRing& rg) {
+  const unsigned cw[8] = {cw0.x, cw0.y, cw0.z, cw0.w, cw1.x, cw1.y, cw1.z, cw1.w};
+  auto item = [&](const int j) {
+    TcItem it;
+    const unsigned c_q = (j & 1) ? (cw[j >> 1] >> 16) : (cw[j >> 1] & 0xffffu);
+    it.n_pass = code_passes(c_q);
+    // fractional index: ki = floor(t) (round-to-nearest of t - 1/2), al = t - ki
+    const float t = Tf[j] + ex;
+    const float u = (t - 0.5f) + kMagic;
+    const float al = t - (u - kMagic);
+    // slot of sample k inside the item's window:  r = ki - window start
+    it.r = (int)__float_as_uint(u) - (int)(kMagicBits + 2u * (unsigned)code_start2(c_q));
+    // weights: P = Ptx_q Prx_m;  W1 = al P (sample k + 1),  W0 = P - W1 (sample k)
+    const float wre = fmaf(pc[j], pr, -ps[j] * pi), wim = fmaf(pc[j], pi, ps[j] * pr);
+    const float w1re = al * wre, w1im = al * wim;
+    it.w0 = pack_half2(wre - w1re, w1im - wim);                    // (Re W0, -Im W0)
+    it.w1 = pack_half2(w1re, -w1im);
+    if (EDGE) {
+      // the term is dropped unless 0 <= k <= K-2 (a pad sample may not lend its neighbour a weight)
+      const int tb_q = __shfl_sync(0xffffffffu, tb_l, min(j, Q - 1));
+      const int ki = (int)(__float_as_uint(u) - kMagicBits);
+      if ((unsigned)(ki + tb_q) > (unsigned)(K - 2)) { it.w0 = 0u; it.w1 = 0u; }
+    }
+    return it;
+  };
+  TcItem cur = item(0);
+#pragma unroll
+  for (int j = 0; j < 16; ++j) {                                 // items in transmit order, q = j
+    TcItem nxt = cur;
+    if (j + 1 < 16) nxt = item(j + 1);
+    int r = cur.r;
+#pragma unroll 1
+    for (int p = 0; p < cur.n_pass; ++p, r -= kTcBlk * kTcPassBlocks) {
+      // the A row of this MMA: slot r holds W0, slot r + 1 holds W1, every other slot 0
+      unsigned v[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) v[i] = 0u;
+#pragma unroll
+      for (int i = -1; i < 8; ++i) {
+        const bool hit = r == i;
+        if (i >= 0) v[i] = hit ? cur.w0 : v[i];
+        if (i < 7) v[i + 1] = hit ? cur.w1 : v[i + 1];
+      }
+      const unsigned buf = rg.a_it & (rg.nab - 1u);
+      // complete the previous A tile (its store has had the placement above to land)
+      tmem_wait_st();
+      tc_fence_before();
+      if (rg.lane0) mbar_arrive(rg.pend);
+      mbar_wait_park(rg.ae0 + 8u * buf, ((rg.a_it >> rg.nab_sh) & 1u) ^ 1u);
+      tc_fence_after();
+      tmem_st8(rg.a_addr0 + buf * kTcACols, v);
+      rg.pend = rg.af0 + 8u * buf;
+      ++rg.a_it;
+    }
+    cur = nxt;
+  }
+}
+
 // Work items: (chunk, tile), tile fastest; every warp role walks the same sequence.
 __global__ void __launch_bounds__(kTcThreads, 1)
 tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ convb, float2* __restrict__ out) {
@@ -154,12 +232,14 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
     const unsigned lane_base = ((unsigned)((warp & 3) * 32)) << 16;
     const unsigned d_addr = tmem + lane_base + (unsigned)(g * N);
     const unsigned a_addr0 = tmem + lane_base + a_col0 + (nab * (unsigned)g) * kTcACols;
-    const unsigned af0 = a_full0 + 8u * (nab * (unsigned)g), ae0 = a_empty0 + 8u * (nab * (unsigned)g);
-    const bool lane0 = lane == 0;
-    const bool lane_has_q = (lane & 15) < P.Q;
-    unsigned a_it = 0, n_done = 0;
-    // a_full barrier of the A tile whose store is in flight; a sink nobody waits on while there is none
-    unsigned pend = smem_u32(&sm.sink);
+    TcGenRing rg;
+    rg.a_it = 0;
+    rg.pend = smem_u32(&sm.sink);
+    rg.nab = nab; rg.nab_sh = nab_sh;
+    rg.ae0 = a_empty0 + 8u * (nab * (unsigned)g); rg.af0 = a_full0 + 8u * (nab * (unsigned)g);
+    rg.a_addr0 = a_addr0;
+    rg.lane0 = lane == 0;
+    unsigned n_done = 0;
 
     for (int work = blockIdx.x; work < n_work; work += gridDim.x, ++n_done) {
       const int tile_i = work % tp.n_tiles, chunk = work / tp.n_tiles;
@@ -181,23 +261,25 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
         ps[j] = sin_approx(ang);
       }
 
-      // the list entry one iteration ahead: header, this lane's window code, receiver position
+      // the list entry one iteration ahead: header, the group's 16 window codes, receiver position
       uint2 hd_n = make_uint2(0u, 0u);
-      unsigned cl_n = 0u;
+      uint4 cw0_n = make_uint4(0u, 0u, 0u, 0u), cw1_n = cw0_n;
       float4 el_n = make_float4(0.f, 0.f, 0.f, 0.f);
       if (td.list_cnt) {
+        const uint4* cp = reinterpret_cast<const uint4*>(tp.codes + ((long long)td.list_off * kTcG + g) * 16);
         hd_n = __ldg(&tp.list[td.list_off]);
-        cl_n = __ldg(&tp.codes[((long long)td.list_off * kTcG + g) * 16 + ql]);
+        cw0_n = __ldg(cp); cw1_n = __ldg(cp + 1);
         el_n = __ldg(&P.elem[hd_n.x]);
       }
       for (int li = 0; li < td.list_cnt; ++li) {
         const uint2 hd = hd_n;
-        const unsigned cl = lane_has_q ? cl_n : 0u;           // window of item (q = lane, m); none beyond Q
+        const uint4 cw0 = cw0_n, cw1 = cw1_n;
         const float4 el = el_n;
         if (li + 1 < td.list_cnt) {
           const long long e = td.list_off + li + 1;
+          const uint4* cp = reinterpret_cast<const uint4*>(tp.codes + (e * kTcG + g) * 16);
           hd_n = __ldg(&tp.list[e]);
-          cl_n = __ldg(&tp.codes[(e * kTcG + g) * 16 + ql]);
+          cw0_n = __ldg(cp); cw1_n = __ldg(cp + 1);
           el_n = __ldg(&P.elem[hd_n.x]);
         }
         if (!((hd.y >> g) & 1u)) continue;                    // no voxel of this group sees receiver m
@@ -208,58 +290,13 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
         cyc -= rintf(cyc);
         const float ang = 6.283185307179586f * cyc;
         const float pr = act ? cos_approx(ang) : 0.f, pi = act ? sin_approx(ang) : 0.f;
-
-#pragma unroll
-        for (int j = 0; j < 16; ++j) {                           // items in transmit order, q = j
-          const unsigned c_q = __shfl_sync(0xffffffffu, cl, j);
-          const int n_pass = code_passes(c_q);
-          // fractional index: ki = floor(t) (round-to-nearest of t - 1/2), al = t - ki
-          const float t = Tf[j] + ex;
-          const float u = (t - 0.5f) + kMagic;
-          const float al = t - (u - kMagic);
-          // slot of sample k inside the item's window:  r = ki - window start
-          int r = (int)__float_as_uint(u) - (int)(kMagicBits + 2u * (unsigned)code_start2(c_q));
-          // weights: P = Ptx_q Prx_m;  W1 = al P (sample k + 1),  W0 = P - W1 (sample k)
-          const float wre = fmaf(pc[j], pr, -ps[j] * pi), wim = fmaf(pc[j], pi, ps[j] * pr);
-          const float w1re = al * wre, w1im = al * wim;
-          unsigned w0 = pack_half2(wre - w1re, w1im - wim);                    // (Re W0, -Im W0)
-          unsigned w1 = pack_half2(w1re, -w1im);
-          if (td.edge) {
-            // reading A6: the term is dropped unless 0 <= k <= K-2 (a pad sample may not lend its
-            // neighbour a weight); only tiles whose windows touch the ends of the record get here
-            const int tb_q = __shfl_sync(0xffffffffu, tb_l, min(j, P.Q - 1));
-            const int ki = (int)(__float_as_uint(u) - kMagicBits);
-            if ((unsigned)(ki + tb_q) > (unsigned)(P.K - 2)) { w0 = 0u; w1 = 0u; }
-          }
-#pragma unroll 1
-          for (int p = 0; p < n_pass; ++p, r -= kTcBlk * kTcPassBlocks) {
-            // the A row of this MMA: slot r holds W0, slot r + 1 holds W1, every other slot 0
-            unsigned v[8];
-#pragma unroll
-            for (int i = 0; i < 8; ++i) v[i] = 0u;
-#pragma unroll
-            for (int i = -1; i < 8; ++i) {
-              const bool hit = r == i;
-              if (i >= 0) v[i] = hit ? w0 : v[i];
-              if (i < 7) v[i + 1] = hit ? w1 : v[i + 1];
-            }
-            const unsigned buf = a_it & (nab - 1u);
-            // complete the previous A tile (its store has had the placement above to land)
-            tmem_wait_st();
-            tc_fence_before();
-            if (lane0) mbar_arrive(pend);
-            mbar_wait_park(ae0 + 8u * buf, ((a_it >> nab_sh) & 1u) ^ 1u);
-            tc_fence_after();
-            tmem_st8(a_addr0 + buf * kTcACols, v);
-            pend = af0 + 8u * buf;
-            ++a_it;
-          }
-        }
+        if (td.edge) tc_gen_receiver<true>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, rg);
+        else tc_gen_receiver<false>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, rg);
       }
       tmem_wait_st();
       tc_fence_before();
-      if (lane0) mbar_arrive(pend);
-      pend = smem_u32(&sm.sink);
+      if (rg.lane0) mbar_arrive(rg.pend);
+      rg.pend = smem_u32(&sm.sink);
 
       // ---- epilogue: D (FP32, TMEM) -> out[frame][voxel] -------------------------------------
       mbar_wait_park(d_full, n_done & 1u);
