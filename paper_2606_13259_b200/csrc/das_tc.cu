@@ -10,29 +10,31 @@ namespace {
 
 // Ring state of one generator warp: the A tiles of its voxel group in tensor memory.
 struct TcGenRing {
-  unsigned a_it;        // passes written so far (slot = a_it mod depth, phase = a_it / depth)
+  unsigned a_it;        // passes this warp set has written (slot = a_it mod depth, phase = a_it / depth)
   unsigned pend;        // a_full barrier of the A tile whose store is in flight (a sink while there is none)
-  unsigned nab, nab_sh; // ring depth and its log2
-  unsigned ae0, af0;    // first a_empty / a_full barrier of the group
-  unsigned a_addr0;     // TMEM address of slot 0 for this warp's lane quarter
+  unsigned nab, nab_sh; // depth of this set's ring and its log2
+  unsigned ae0, af0;    // first a_empty / a_full barrier of this set's ring
+  unsigned a_addr0;     // TMEM address of the ring's slot 0 for this warp's lane quarter
   bool lane0;
 };
 
 // One (q, m) item of a generator thread: the two packed weights, the slot of sample k, the passes.
 struct TcItem { unsigned w0, w1; int r, n_pass; };
 
-// All 16 items of one receiver for one voxel row.  cw[] holds the 16 window codes of the group
+// The items (q = kTcSets j + h, m) of one receiver for one voxel row.  cw[] holds the 16 window codes of the group
 // (two per word, loaded with one address for the whole warp: no shuffle in the chain).  The item
 // math of q + 1 is written before the stores of q, so that it fills the latency of the
 // store / barrier sequence.  EDGE: the tile's windows touch the ends of the record (reading A6).
 template <bool EDGE>
-__device__ __forceinline__ void tc_gen_receiver(const float (&Tf)[16], const float (&pc)[16], const float (&ps)[16],
+__device__ __forceinline__ void tc_gen_receiver(const float (&Tf)[kTcQPerSet], const float (&pc)[kTcQPerSet], const float (&ps)[kTcQPerSet], const int h,
                                                 const float ex, const float pr, const float pi, const uint4 cw0,
                                                 const uint4 cw1, const int tb_l, const int Q, const int K, TcGenRing& rg) {
   const unsigned cw[8] = {cw0.x, cw0.y, cw0.z, cw0.w, cw1.x, cw1.y, cw1.z, cw1.w};
   auto item = [&](const int j) {
     TcItem it;
-    const unsigned c_q = (j & 1) ? (cw[j >> 1] >> 16) : (cw[j >> 1] & 0xffffu);
+    const int q = kTcSets * j + h;                                   // static when kTcSets == 1
+    const unsigned cww = cw[kTcSets == 2 ? j : (j >> 1)];
+    const unsigned c_q = (q & 1) ? (cww >> 16) : (cww & 0xffffu);
     it.n_pass = code_passes(c_q);
     // fractional index: ki = floor(t) (round-to-nearest of t - 1/2), al = t - ki
     const float t = Tf[j] + ex;
@@ -47,7 +49,7 @@ __device__ __forceinline__ void tc_gen_receiver(const float (&Tf)[16], const flo
     it.w1 = pack_half2(w1re, -w1im);
     if (EDGE) {
       // the term is dropped unless 0 <= k <= K-2 (a pad sample may not lend its neighbour a weight)
-      const int tb_q = __shfl_sync(0xffffffffu, tb_l, min(j, Q - 1));
+      const int tb_q = __shfl_sync(0xffffffffu, tb_l, min(q, Q - 1));
       const int ki = (int)(__float_as_uint(u) - kMagicBits);
       if ((unsigned)(ki + tb_q) > (unsigned)(K - 2)) { it.w0 = 0u; it.w1 = 0u; }
     }
@@ -55,9 +57,9 @@ __device__ __forceinline__ void tc_gen_receiver(const float (&Tf)[16], const flo
   };
   TcItem cur = item(0);
 #pragma unroll
-  for (int j = 0; j < 16; ++j) {                                 // items in transmit order, q = j
+  for (int j = 0; j < kTcQPerSet; ++j) {                         // this set's items in transmit order
     TcItem nxt = cur;
-    if (j + 1 < 16) nxt = item(j + 1);
+    if (j + 1 < kTcQPerSet) nxt = item(j + 1);
     int r = cur.r;
 #pragma unroll 1
     for (int p = 0; p < cur.n_pass; ++p, r -= kTcBlk * kTcPassBlocks) {
@@ -123,8 +125,8 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
   const unsigned nab = (unsigned)tp.a_bufs, nab_sh = (unsigned)tp.a_shift;   // A ring depth (power of two)
   // The accumulators start from zero and the epilogue leaves them zero again, so every MMA accumulates
   // and no MMA has to be the first (kTcIssuers warps of a group need no order between them).
-  if (warp < kTcGenWarps) {
-    const unsigned d0 = tmem + (((unsigned)((warp & 3) * 32)) << 16) + (unsigned)((warp >> 2) * N);
+  if (warp < kTcGenWarps && ((warp >> 2) % kTcSets) == 0) {
+    const unsigned d0 = tmem + (((unsigned)((warp & 3) * 32)) << 16) + (unsigned)((warp / (4 * kTcSets)) * N);
     for (int c0 = 0; c0 < N; c0 += 8) tmem_st8_zero(d0 + (unsigned)c0);
     tmem_wait_st();
   }
@@ -181,7 +183,10 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
     const unsigned af0 = a_full0 + 8u * (nab * (unsigned)g), ae0 = a_empty0 + 8u * (nab * (unsigned)g);
     // descriptor of a B tile at shared address 0: LBO = one slab (the two K chunks), SBO = 128 B
     const unsigned long long desc0 = tc_smem_desc(0u, slab, 128);
-    unsigned s = 0, ph = 0, a_it = 0, n_done = 0;
+    // every generator warp set has its own A ring (nab / kTcSets slots): the passes of the items q = kTcSets j + h
+    const unsigned nas = nab / kTcSets, nas_sh = nab_sh - (kTcSets == 2 ? 1u : 0u);
+    unsigned s = 0, ph = 0, n_done = 0;
+    unsigned a_its[kTcSets] = {};
     for (int work = blockIdx.x; work < n_work; work += gridDim.x, ++n_done) {
       const int tile_i = work % tp.n_tiles;
       const TcTile td = tp.tiles[tile_i];
@@ -201,20 +206,23 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
           const unsigned info = __shfl_sync(0xffffffffu, info_l, q);
           const int np = (int)(info & 3u);
           if ((q % kTcIssuers) != par) {                      // the other warp's item: count its ring slots
-            a_it += (unsigned)np;
+            a_its[q % kTcSets] += (unsigned)np;
           } else {
           mbar_wait_park(b_full0 + 8 * s, ph);                 // also keeps an idle group in step with the ring
           if (np) {
             unsigned long long desc = desc0 + (unsigned long long)(((stage0 + s * stage_bytes) >> 4) + (info >> 2));
+            const unsigned set = (unsigned)(q % kTcSets);
+            unsigned a_it = a_its[kTcSets == 2 ? (q & 1) : 0];
             for (int p = 0; p < np; ++p, ++a_it, desc += (unsigned long long)((kTcPassBlocks * slab) >> 4)) {
-              const unsigned buf = a_it & (nab - 1u);
-              mbar_wait_park(af0 + 8u * buf, (a_it >> nab_sh) & 1u);
+              const unsigned buf = set * nas + (a_it & (nas - 1u));
+              mbar_wait_park(af0 + 8u * buf, (a_it >> nas_sh) & 1u);
               tc_fence_after();
               if (tc_elect()) {
                 tc_mma_ts(d_tmem, a_tmem0 + buf * kTcACols, desc, idesc, 1u);
                 tc_commit(ae0 + 8u * buf);                     // A buffer free once this MMA has read it
               }
             }
+            a_its[kTcSets == 2 ? (q & 1) : 0] = a_it;
             if (tc_elect()) tc_commit(b_empty0 + 8 * s);       // this group is done with the stage
           } else if (lane == 0) {
             mbar_arrive(b_empty0 + 8 * s);                     // nothing to read: release at once
@@ -227,7 +235,8 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
     }
   } else {
     // ===================================== GENERATORS =========================================
-    const int g = warp >> 2;                                  // voxel group = depth inside the tile
+    const int g = warp / (4 * kTcSets);                       // voxel group = depth inside the tile
+    const int h = (warp >> 2) % kTcSets;                      // warp set: it takes the transmits q = kTcSets j + h
     const int row = (warp & 3) * 32 + lane;                   // MMA row = TMEM lane (quarter warp % 4)
     const unsigned lane_base = ((unsigned)((warp & 3) * 32)) << 16;
     const unsigned d_addr = tmem + lane_base + (unsigned)(g * N);
@@ -235,9 +244,12 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
     TcGenRing rg;
     rg.a_it = 0;
     rg.pend = smem_u32(&sm.sink);
-    rg.nab = nab; rg.nab_sh = nab_sh;
-    rg.ae0 = a_empty0 + 8u * (nab * (unsigned)g); rg.af0 = a_full0 + 8u * (nab * (unsigned)g);
-    rg.a_addr0 = a_addr0;
+    rg.nab = nab / kTcSets; rg.nab_sh = nab_sh - (kTcSets == 2 ? 1u : 0u);
+    rg.ae0 = a_empty0 + 8u * (nab * (unsigned)g + rg.nab * (unsigned)h); rg.af0 = a_full0 + 8u * (nab * (unsigned)g + rg.nab * (unsigned)h);
+    rg.a_addr0 = a_addr0 + rg.nab * (unsigned)h * kTcACols;
+    // epilogue columns of this set: half of D each when a half is a whole number of 16-column loads
+    const bool split = kTcSets == 2 && (N % 32) == 0;
+    const int col_lo = split ? h * (N / 2) : 0, col_hi = split ? col_lo + N / 2 : (h == 0 ? N : 0);
     rg.lane0 = lane == 0;
     unsigned n_done = 0;
 
@@ -248,10 +260,10 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
       const int tb_l = __ldg(&tp.tbase[(long long)tile_i * P.Q + ql]);
 
       // per-(q, n) part in FP64: reduced transmit delay and transmit phase factor
-      float Tf[16], pc[16], ps[16];
+      float Tf[kTcQPerSet], pc[kTcQPerSet], ps[kTcQPerSet];
 #pragma unroll
-      for (int j = 0; j < 16; ++j) {
-        const int qq = min(j, P.Q - 1);
+      for (int j = 0; j < kTcQPerSet; ++j) {
+        const int qq = min(kTcSets * j + h, P.Q - 1);
         const double T = tc_T(P, vx, qq);
         Tf[j] = (float)(T - (double)__ldg(&tp.tbase[(long long)tile_i * P.Q + qq]));
         double cyc = tp.phase0 + tp.ratio * T;
@@ -290,8 +302,8 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
         cyc -= rintf(cyc);
         const float ang = 6.283185307179586f * cyc;
         const float pr = act ? cos_approx(ang) : 0.f, pi = act ? sin_approx(ang) : 0.f;
-        if (td.edge) tc_gen_receiver<true>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, rg);
-        else tc_gen_receiver<false>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, rg);
+        if (td.edge) tc_gen_receiver<true>(Tf, pc, ps, h, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, rg);
+        else tc_gen_receiver<false>(Tf, pc, ps, h, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, rg);
       }
       tmem_wait_st();
       tc_fence_before();
@@ -303,7 +315,7 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
       tc_fence_after();
       const long long vox = ((long long)vx.ix * P.ny + vx.iy) * P.nz + vx.iz;
       float2* dst = out + (long long)chunk * tp.Bc * n_vox + vox;
-      for (int c0 = 0; c0 < N; c0 += 16) {
+      for (int c0 = col_lo; c0 < col_hi; c0 += 16) {
         float v[16];
         tmem_ld16(d_addr + (unsigned)c0, v);
         tmem_wait_ld();

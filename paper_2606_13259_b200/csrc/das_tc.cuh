@@ -51,10 +51,13 @@ constexpr int kTcMaxStages = 16;            // upper bound of the shared-memory 
 constexpr int kTcMinStages = 2;
 constexpr int kTcPadBlocks = 16;            // zero k-blocks before and after every (m, q) row
 constexpr int kTcMaxStageBlocks = 16;       // largest window (k-blocks) one stage can hold
-constexpr int kTcGenWarps = 4 * kTcG;
+constexpr int kTcSets = 1;                   // generator warp sets per voxel group (2: even / odd transmits, each with its own
+                                             // A ring; correct, but 119.6 ms against 110.7 ms at the headline: 72 registers
+                                             // per thread with spills and rings of two slots)
+constexpr int kTcQPerSet = 16 / kTcSets;
+constexpr int kTcGenWarps = 4 * kTcSets * kTcG;
 constexpr int kTcIssuers = 1;                // MMA issuer warps per voxel group (2 share the items by the parity of q:
-                                             // correct, but measured 152 ms against 130 ms per 64-frame batch at the
-                                             // headline: the extra warps take issue slots from the generators)
+                                             // correct, measured 109.8 ms against 110.7 ms per 64-frame batch: no gain)
 constexpr int kTcSvcWarps = 1 + kTcIssuers * kTcG;   // TMA producer + the MMA issuers
 constexpr int kTcThreads = (kTcSvcWarps + kTcGenWarps) * 32;
 constexpr int kTcTmemCols = 512;

@@ -210,6 +210,7 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
   if (const char* ev = getenv("DAS_TC_ABUFS")) dv.a_shift = std::min(3, std::max(0, atoi(ev)));   // tuning sweeps only
   while (dv.a_shift > 0 && kTcG * 2 * Bc + kTcG * (1 << dv.a_shift) * kTcACols > kTcTmemCols) --dv.a_shift;
   dv.a_bufs = 1 << dv.a_shift;
+  if (dv.a_bufs < kTcSets) return refuse_free("tensor memory cannot hold an A ring per generator warp set");
   // The ring only has to cover the L2 latency of a window: measured flat from 4 to 8 stages at the
   // headline, slower at 16 (the CTAs drift apart and L2 holds fewer of their shared windows).
   dv.n_stages = 6;
