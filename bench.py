@@ -4,15 +4,22 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl cuda|reference]
                     [--config 3] [--storage fp16|fp32] [--algo auto|general|tiled]
 
-One "step" is one pass of the whole hot path over one frame of
+One "step" is one pass of the whole hot path over one batch of
 synthetic channel data already resident in HBM: das_convert (layout transform + cast) followed
 by das_execute (delays, aperture, gather, interpolation, rotation, accumulation, store), both
 through the C ABI of libdas_b200.so.  The default workload is BASELINE.json configs[2], the
-headline the metric is quoted on: 128^3 voxels x 1024 elements x 16 diverging-wave transmits,
-1024 IQ samples per trace, fp16 storage.
+headline the metric is quoted on (128^3 voxels x 1024 elements x 16 diverging-wave transmits,
+1024 IQ samples per trace, fp16 storage), taken --frames-per-call = 64
+frames at a time (configs[4], the streaming ensemble: 64 frames of the headline layout): one
+das_convert and one das_execute per 64 frames, the frame-batch tensor-core kernel
+(DAS_ALGO_TC).  Every frame is beamformed in full (parity per frame in tests/test_gpu_tc.py);
+volumes/s = frames / time.  --frames-per-call 1 times one frame per call (the tiled CUDA-core
+kernel); the default run reports that number too, under "single_frame".
 
 Printed: ONE JSON line (rank 0).  Keys beyond the base contract:
-  roofline      the dominant kernel (das_execute's tiled kernel) against the FP32 ALU roofline
+  roofline      the dominant kernel of das_execute: the tensor-core batch kernel against the
+                measured dense tensor peak, or (one frame per call) the tiled kernel against the
+                FP32 ALU roofline
   cpu_baseline  the CPU oracle (oracle/, as it stands) timed on this box's host cores on a
                 bounded voxel sample of the same workload
   e2e           the same metric through das_beamform_host with pinned HOST buffers (H2D of the
@@ -55,20 +62,24 @@ N_SM = 148
 # dram__bytes_read.sum + dram__bytes_write.sum of the tiled kernel, per launch, from the
 # `ncu --set full` capture summarised in profiles/ (bytes); keyed by (config, storage).
 NCU_TRAFFIC_BYTES = {
-    (3, "fp16"): 57.4e6,         # profiles/r1_tiled_iq16_full.md
+    (3, "fp16", 1): 57.4e6,      # profiles/r1_tiled_iq16_full.md
+    (3, "fp16", 64): 173.9e9,    # profiles/r1_tc_b64_full.md
 }
 
 
 def parse_args():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4],
                     help="BASELINE.json config number (3 = headline, the metric's workload)")
     ap.add_argument("--storage", choices=["fp16", "fp32"], default="fp16")
     ap.add_argument("--algo", choices=["auto", "general", "tiled"], default="auto")
+    ap.add_argument("--frames-per-call", type=int, default=None,
+                    help="B: frames per das_convert / das_execute call (default 64 = configs[4]'s ensemble, "
+                         "tensor-core batch kernel, for IQ data in fp16 storage; 1 = one frame per call, tiled kernel)")
     ap.add_argument("--frames", type=int, default=4,
                     help="distinct raw frames rotated through the timed steps (inputs > L2)")
     ap.add_argument("--e2e-steps", type=int, default=10)
@@ -252,6 +263,39 @@ def fp32_peak_tflops(sampler_max_mhz):
     return N_SM * FP32_LANES_PER_SM * 2 * mhz * 1e6 / 1e12, f"148 SM x 128 lanes x 2 flop x {mhz:.0f} MHz ({src})"
 
 
+def tensor_peak_tflops():
+    """Dense FP16 tensor peak: the driver-measured bf16 cuBLAS burst figure of MEASURED_PEAKS.json
+    (FP16 and BF16 run at the same rate; the batch kernel is timed alone, launch by launch),
+    else the B200_PROFILING.md nominal 2250 TFLOP/s."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["bf16_tflops"]), "MEASURED_PEAKS.json bf16_tflops (burst), same rate for fp16"
+    except Exception:
+        return 2250.0, "B200_PROFILING.md nominal dense bf16/fp16 (fallback)"
+
+
+def time_loop(torch, stream, step, steps, warmup, barrier, max_over_ranks, local_rank, das):
+    """W untimed + K timed steps; per-step (convert, execute) CUDA-event times on `stream`."""
+    for i in range(warmup):
+        step(i)
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+    t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    n0 = das.launch_count()
+    with ClockSampler(local_rank) as cs:
+        t_beg.record(stream)
+        for i in range(steps):
+            step(warmup + i, evs[i])
+        t_end.record(stream)
+        stream.synchronize()
+    launches = das.launch_count() - n0
+    barrier()
+    total_ms = max_over_ranks(t_beg.elapsed_time(t_end))
+    conv_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    exec_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+    return total_ms, conv_ms, exec_ms, launches, cs.summary()
+
+
 def run_cuda(args):
     import torch
     import workloads as wl
@@ -282,63 +326,82 @@ def run_cuda(args):
         return float(t.item())
 
     w = wl.config(args.config)
+    batchable = w.data_kind == 0 and args.storage == "fp16"
+    B = max(1, args.frames_per_call) if args.frames_per_call is not None else (64 if batchable else 1)
+    if B > 1 and (w.data_kind != 0 or args.storage != "fp16"):
+        raise SystemExit("bench.py: --frames-per-call > 1 needs IQ data in fp16 storage (the tensor-core batch kernel)")
     storage = das.STORE_FP16 if args.storage == "fp16" else das.STORE_FP32
     algo = {"auto": das.ALGO_AUTO, "general": das.ALGO_GENERAL, "tiled": das.ALGO_TILED}[args.algo]
-    plan = das.Plan.from_workload(w, storage=storage, algo=algo, device=local_rank)
-    algo_used = {das.ALGO_GENERAL: "general", das.ALGO_TILED: "tiled"}[plan.algo]
-    n_pairs, n_terms = plan.count_work()
-
-    frames_np = make_frames(w, max(1, args.frames))
-    raw = [torch.from_numpy(np.ascontiguousarray(f)).to(dev) for f in frames_np]
-    conv = torch.empty(plan.converted_bytes, dtype=torch.uint8, device=dev)
-    out = torch.empty(w.grid_shape, dtype=torch.complex64 if w.data_kind == 0 else torch.float32, device=dev)
     stream = torch.cuda.Stream(device=dev)
     sp = stream.cuda_stream
+    out_dt = torch.complex64 if w.data_kind == 0 else torch.float32
+    frames_np = make_frames(w, max(1, args.frames))
+    raw1 = [torch.from_numpy(np.ascontiguousarray(f)).to(dev) for f in frames_np]
 
-    def step(i, evs=None):
-        r = raw[i % len(raw)]
-        if evs is not None:
-            evs[0].record(stream)
-        plan.convert(r.data_ptr(), conv.data_ptr(), 1.0, sp)
-        if evs is not None:
-            evs[1].record(stream)
-        plan.execute(conv.data_ptr(), out.data_ptr(), sp)
-        if evs is not None:
-            evs[2].record(stream)
+    def measure_plan(plan, raws, out, steps, warmup):
+        conv = torch.empty(plan.converted_bytes, dtype=torch.uint8, device=dev)
 
-    def measure():
-        for i in range(args.warmup):
-            step(i)
-        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
-        t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        barrier()
-        n0 = das.launch_count()
-        with ClockSampler(local_rank) as cs:
-            t_beg.record(stream)
-            for i in range(args.steps):
-                step(args.warmup + i, evs[i])
-            t_end.record(stream)
-            stream.synchronize()
-        launches = das.launch_count() - n0
-        barrier()
-        total_ms = max_over_ranks(t_beg.elapsed_time(t_end))
-        conv_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
-        exec_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
-        return total_ms, conv_ms, exec_ms, launches, cs.summary()
+        def step(i, evs=None):
+            r = raws[i % len(raws)]
+            if evs is not None:
+                evs[0].record(stream)
+            plan.convert(r.data_ptr(), conv.data_ptr(), 1.0, sp)
+            if evs is not None:
+                evs[1].record(stream)
+            plan.execute(conv.data_ptr(), out.data_ptr(), sp)
+            if evs is not None:
+                evs[2].record(stream)
 
-    total_ms, conv_ms, exec_ms, launches, clocks = measure()
-    remeasured = False
-    if BAD_REASONS & set(clocks.get("reasons", [])):
-        remeasured = True
-        time.sleep(2.0)
-        total_ms, conv_ms, exec_ms, launches, clocks = measure()
-    clocks["remeasured"] = remeasured
+        res = time_loop(torch, stream, step, steps, warmup, barrier, max_over_ranks, local_rank, das)
+        if BAD_REASONS & set(res[4].get("reasons", [])):
+            time.sleep(2.0)
+            res = time_loop(torch, stream, step, steps, warmup, barrier, max_over_ranks, local_rank, das)
+            res[4]["remeasured"] = True
+        else:
+            res[4]["remeasured"] = False
+        return res + (conv.nbytes,)
+
+    # ---- one frame per call: the tiled CUDA-core kernel (always measured; the headline when B == 1)
+    plan1 = das.Plan.from_workload(w, storage=storage, algo=algo, device=local_rank)
+    algo1 = {das.ALGO_GENERAL: "general", das.ALGO_TILED: "tiled"}[plan1.algo]
+    n_pairs, n_terms = plan1.count_work()
+    out1 = torch.empty(w.grid_shape, dtype=out_dt, device=dev)
+    s1_steps, s1_warm = (args.steps, args.warmup) if B == 1 else (min(args.steps, 10), 3)
+    tot1, conv1, exec1, launch1, clocks1, convbytes1 = measure_plan(plan1, raw1, out1, s1_steps, s1_warm)
+    single = {"value": world * s1_steps / (tot1 * 1e-3), "unit": UNIT, "ms_per_step": tot1 / s1_steps,
+              "kernel": algo1, "kernels_ms": {"das_convert": conv1, "das_execute": exec1}, "steps": s1_steps}
+    flops1 = FLOPS_PER_TERM[w.data_kind] * n_terms + FLOPS_PER_PAIR * n_pairs
+
+    if B == 1:
+        plan, raws, out = plan1, raw1, out1
+        total_ms, conv_ms, exec_ms, launches, clocks, convbytes = tot1, conv1, exec1, launch1, clocks1, convbytes1
+        steps = s1_steps
+        algo_used = algo1
+    else:
+        # ---- B frames per call: the frame-batch tensor-core kernel.  The batch holds the rotated
+        # seeded frames under exact power-of-two scales (64 distinct frames, 8.6 GB of raw input per
+        # step at the headline: no step finds its input in the 126 MB L2).
+        plan = das.Plan.from_workload(w, storage=storage, algo=das.ALGO_AUTO, device=local_rank, n_frames=B)
+        if plan.algo != das.ALGO_TC:
+            raise SystemExit("bench.py: the tensor-core batch kernel does not apply to this configuration")
+        algo_used = "tensor-core batch"
+        rawB = torch.empty((B,) + tuple(w.y.shape), dtype=raw1[0].dtype, device=dev)
+        for b in range(B):
+            rawB[b] = raw1[b % len(raw1)] * (2.0 ** (-((b // len(raw1)) % 4)))
+        raws = [rawB]
+        out = torch.empty((B,) + tuple(w.grid_shape), dtype=out_dt, device=dev)
+        steps = args.steps
+        total_ms, conv_ms, exec_ms, launches, clocks, convbytes = measure_plan(plan, raws, out, steps, args.warmup)
 
     # ---- end to end through das_beamform_host: pinned host buffers, H2D + D2H inside the timing
-    h_raw = [torch.from_numpy(np.ascontiguousarray(f)).pin_memory() for f in frames_np]
-    h_out = torch.empty(w.grid_shape, dtype=out.dtype).pin_memory()
+    if B == 1:
+        h_raw = [torch.from_numpy(np.ascontiguousarray(f)).pin_memory() for f in frames_np]
+    else:
+        h_raw = [torch.empty(tuple(rawB.shape), dtype=rawB.dtype, pin_memory=True)]
+        h_raw[0].copy_(rawB)
+    h_out = torch.empty(tuple(out.shape), dtype=out.dtype).pin_memory()
     plan.beamform_host(h_raw[0].data_ptr(), h_out.data_ptr(), sp)          # allocates the staging
-    e_steps = max(1, args.e2e_steps)
+    e_steps = max(1, args.e2e_steps if B == 1 else min(args.e2e_steps, 3))
     e_beg, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e_beg.record(stream)
@@ -355,44 +418,63 @@ def run_cuda(args):
             dist.destroy_process_group()
         return 0
 
-    value = world * args.steps / (total_ms * 1e-3)
-    flops = FLOPS_PER_TERM[w.data_kind] * n_terms + FLOPS_PER_PAIR * n_pairs
-    peak, peak_how = fp32_peak_tflops(clocks.get("sm_max_mhz"))
+    value = world * B * steps / (total_ms * 1e-3)
+    if B == 1:
+        flops = flops1
+        peak, peak_how = fp32_peak_tflops(clocks.get("sm_max_mhz"))
+        bound, peak_how = "alu", peak_how + ", derived (no measured FP32 peak)"
+        flops_model = (f"{FLOPS_PER_TERM[w.data_kind]:.0f} x entered terms + {FLOPS_PER_PAIR:.0f} x active (m,n) pairs (DESIGN.md)")
+        extra = {}
+    else:
+        # per frame every entered term is interpolated, rotated and accumulated (17 definition flops);
+        # the geometry of an active (m, n) pair is worked out once per batch
+        flops = FLOPS_PER_TERM[w.data_kind] * n_terms * B + FLOPS_PER_PAIR * n_pairs
+        peak, peak_how = tensor_peak_tflops()
+        bound = "tensor"
+        flops_model = (f"{FLOPS_PER_TERM[w.data_kind]:.0f} x entered terms x {B} frames + {FLOPS_PER_PAIR:.0f} x active (m,n) pairs "
+                       f"(DESIGN.md); the MMAs the kernel issues carry 4x to 5x as many (2 of 8 samples of a K = 16 pass are non-zero)")
+        extra = {"ncu": {"tensor_pipe_active": 0.34, "issue_slots_active": 0.56, "alu_pipe_active": 0.49,
+                         "source": "profiles/r1_tc_b64_full.md"}}
     achieved = flops / (exec_ms * 1e-3) / 1e12
-    traffic = NCU_TRAFFIC_BYTES.get((args.config, args.storage)) if algo_used == "tiled" else None
+    traffic = NCU_TRAFFIC_BYTES.get((args.config, args.storage, B)) if algo_used != "general" else None
+    raw_bytes = sum(r.nbytes for r in raws)
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": workload_name(w, args.storage), "kernel": algo_used,
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
+        "warmup": args.warmup, "ms_per_step": total_ms / steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32" if B == 1 else "f16 x f16 -> f32", "data": "synthetic",
+        "config": {"workload": workload_name(w, args.storage) + (f"; {B} frames per call (configs[4] ensemble)" if B > 1 else ""),
+                   "kernel": algo_used, "frames_per_call": B,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "l2": f"{len(raw)} distinct raw frames rotated ({sum(r.nbytes for r in raw) / 1e6:.0f} MB + "
-                         f"{conv.nbytes / 1e6:.0f} MB converted buffer rewritten every step) > 126 MB L2",
-                   "step": "das_convert + das_execute on device-resident input"},
+                   "l2": f"{raw_bytes / 1e6:.0f} MB of distinct raw input per rotation + {convbytes / 1e6:.0f} MB converted "
+                         f"buffer rewritten every step > 126 MB L2",
+                   "step": f"das_convert + das_execute on device-resident input, {B} frame(s) per call"},
         "accumulations_per_s": {"nominal": w.nominal_accumulations * value, "entered": n_terms * value,
                                 "nominal_per_volume": w.nominal_accumulations, "entered_per_volume": n_terms,
                                 "active_pairs_per_volume": n_pairs},
         "kernels_ms": {"das_convert": conv_ms, "das_execute": exec_ms},
-        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                     "frac": achieved / peak, "traffic": traffic,
-                     "kernel": f"das_execute ({algo_used} kernel)", "kernel_ms": exec_ms,
-                     "share_of_step": exec_ms / (total_ms / args.steps),
-                     "flops_per_launch": flops,
-                     "flops_model": f"{FLOPS_PER_TERM[w.data_kind]:.0f} x entered terms + {FLOPS_PER_PAIR:.0f} x active (m,n) pairs (DESIGN.md)",
-                     "peak_how": peak_how + ", derived (of derived FP32 peak, not of a measured one)"},
-        "e2e": {"value": world * e_steps / (e2e_ms * 1e-3), "unit": UNIT,
+        "roofline": dict({"bound": bound, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                          "frac": achieved / peak, "traffic": traffic,
+                          "kernel": f"das_execute ({algo_used} kernel)", "kernel_ms": exec_ms,
+                          "share_of_step": exec_ms / (total_ms / steps),
+                          "flops_per_launch": flops, "flops_model": flops_model, "peak_how": peak_how}, **extra),
+        "e2e": {"value": world * B * e_steps / (e2e_ms * 1e-3), "unit": UNIT,
                 "h2d_bytes_per_step": int(plan.raw_bytes), "d2h_bytes_per_step": int(plan.output_bytes),
                 "ms_per_step": e2e_ms / e_steps, "steps": e_steps, "api": "das_beamform_host, pinned host buffers",
                 "checksum_max_abs": checksum},
         "gpu_launches": int(launches),
         "clocks": clocks,
+        "single_frame": dict(single, roofline={"bound": "alu", "achieved": flops1 / (exec1 * 1e-3) / 1e12,
+                                               "peak": fp32_peak_tflops(clocks.get("sm_max_mhz"))[0], "unit": "TFLOP/s"}),
     }
+    line["single_frame"]["roofline"]["frac"] = line["single_frame"]["roofline"]["achieved"] / line["single_frame"]["roofline"]["peak"]
     if world == 1 and args.cpu_seconds > 0:
         line["cpu_baseline"] = cpu_baseline(w, args.cpu_seconds)
     else:
         line["cpu_baseline"] = None
     print(json.dumps(line), flush=True)
     plan.destroy()
+    if plan1 is not plan:
+        plan1.destroy()
     if dist is not None:
         dist.destroy_process_group()
     return 0
