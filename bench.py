@@ -62,8 +62,8 @@ N_SM = 148
 # dram__bytes_read.sum + dram__bytes_write.sum of the tiled kernel, per launch, from the
 # `ncu --set full` capture summarised in profiles/ (bytes); keyed by (config, storage).
 NCU_TRAFFIC_BYTES = {
-    (3, "fp16", 1): 57.4e6,      # profiles/r1_tiled_iq16_full.md
-    (3, "fp16", 64): 173.9e9,    # profiles/r1_tc_b64_full.md
+    (3, "fp16", 1): 57.05e6,     # profiles/r1_tiled_v3_iq16_full.md
+    (3, "fp16", 64): 174.8e9,    # profiles/r1_tc_b64_full.md
 }
 
 
