@@ -110,7 +110,7 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
   if (tid == 0) {
     for (int s = 0; s < kTcMaxStages; ++s) { mbar_init(b_full0 + 8 * s, 1); mbar_init(b_empty0 + 8 * s, kTcG); }
     for (int i = 0; i < kTcMaxABufs * kTcG; ++i) { mbar_init(a_full0 + 8 * i, 4); mbar_init(a_empty0 + 8 * i, 1); }
-    mbar_init(d_full, kTcG * kTcIssuers);
+    mbar_init(d_full, kTcG);
     mbar_init(d_empty, kTcGenWarps);
     mbar_init(smem_u32(&sm.sink), 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -124,7 +124,7 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
   const unsigned a_col0 = (unsigned)(kTcG * N);
   const unsigned nab = (unsigned)tp.a_bufs, nab_sh = (unsigned)tp.a_shift;   // A ring depth (power of two)
   // The accumulators start from zero and the epilogue leaves them zero again, so every MMA accumulates
-  // and no MMA has to be the first (kTcIssuers warps of a group need no order between them).
+  // and no MMA has to be the first of its tile.
   if (warp < kTcGenWarps && ((warp >> 2) % kTcSets) == 0) {
     const unsigned d0 = tmem + (((unsigned)((warp & 3) * 32)) << 16) + (unsigned)((warp / (4 * kTcSets)) * N);
     for (int c0 = 0; c0 < N; c0 += 8) tmem_st8_zero(d0 + (unsigned)c0);
@@ -136,8 +136,11 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
 
   if (warp == kTcGenWarps) {
     // ===================================== TMA PRODUCER =======================================
-    // lane q works out the window of item (q, m): the union over the voxel groups; lane 0 issues
+    // A stage holds the windows of kTcQS consecutive transmits of one receiver (one barrier round
+    // per kTcQS items).  Lane q works out the window of item (q, m), the union over the voxel groups,
+    // and issues its own bulk copy; lane 0 waits for the stage and posts the byte count.
     unsigned s = 0, ph = 0;                                  // stage and its phase parity
+    const bool has_q = lane < P.Q;
     for (int work = blockIdx.x; work < n_work; work += gridDim.x) {
       const int tile_i = work % tp.n_tiles, chunk = work / tp.n_tiles;
       const TcTile td = tp.tiles[tile_i];
@@ -151,19 +154,18 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
         tc_union_window(tp.codes + e * kTcG * 16 + ql, wlo, wn);
         // byte offset of the window inside the chunk and its length, per lane = q
         const long long src_l = ((long long)hd.x * P.Q * tp.KBp + kTcPadBlocks + (long long)ql * tp.KBp + tb4 + wlo) * (long long)slab;
-        const unsigned bytes_l = (unsigned)wn * slab;
-        for (int q = 0; q < P.Q; ++q) {
-          const long long src = __shfl_sync(0xffffffffu, src_l, q);
-          const unsigned bytes = __shfl_sync(0xffffffffu, bytes_l, q);
+        const unsigned bytes_l = has_q ? (unsigned)wn * slab : 0u;
+        for (int q0 = 0; q0 < P.Q; q0 += kTcQS) {
+          const bool mine = lane >= q0 && lane < q0 + kTcQS;
+          const unsigned total = __reduce_add_sync(0xffffffffu, mine ? bytes_l : 0u);
           if (lane == 0) {
             mbar_wait_park(b_empty0 + 8 * s, ph ^ 1u);
-            if (bytes) {
-              mbar_arrive_expect_tx(b_full0 + 8 * s, bytes);
-              tma_bulk_g2s(stage0 + s * stage_bytes, base + src, bytes, b_full0 + 8 * s);
-            } else {
-              mbar_arrive(b_full0 + 8 * s);
-            }
+            if (total) mbar_arrive_expect_tx(b_full0 + 8 * s, total);
+            else mbar_arrive(b_full0 + 8 * s);
           }
+          __syncwarp();
+          if (mine && bytes_l)
+            tma_bulk_g2s(stage0 + (s * kTcQS + (unsigned)(lane - q0)) * stage_bytes, base + src_l, bytes_l, b_full0 + 8 * s);
           if (++s == (unsigned)tp.n_stages) { s = 0; ph ^= 1u; }
           __syncwarp();
         }
@@ -171,22 +173,19 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
     }
   } else if (warp > kTcGenWarps) {
     // ===================================== MMA ISSUERS ========================================
-    // kTcIssuers warps per voxel group share the items (q, m) by the parity of q.  The issue loop is
-    // a serial chain (wait -> MMA -> commit) whose latency bounds the MMA rate of a group, so it is
-    // kept as short as it can be: lane q prepares item (q, m) (passes, offset of the group's window
-    // inside the staged one), every lane runs the same scalar loop (no divergence, one shuffle per
-    // item), and only the tcgen05 instructions sit under an elected lane.
-    const int g = (warp - kTcGenWarps - 1) / kTcIssuers, par = (warp - kTcGenWarps - 1) % kTcIssuers;
+    // One warp per voxel group.  The issue loop is a serial chain (wait -> MMA -> commit) whose
+    // latency bounds the MMA rate of a group, so it is kept as short as it can be: lane q prepares
+    // item (q, m) (passes, offset of the group's window inside the staged one), every lane runs the
+    // same scalar loop (no divergence, one shuffle per item), only the tcgen05 instructions sit
+    // under an elected lane, and the stage barriers are visited once per kTcQS items.
+    const int g = warp - kTcGenWarps - 1;
     const unsigned idesc = tc_idesc(N);
     const unsigned d_tmem = tmem + (unsigned)(g * N);
     const unsigned a_tmem0 = tmem + a_col0 + (nab * (unsigned)g) * kTcACols;
     const unsigned af0 = a_full0 + 8u * (nab * (unsigned)g), ae0 = a_empty0 + 8u * (nab * (unsigned)g);
     // descriptor of a B tile at shared address 0: LBO = one slab (the two K chunks), SBO = 128 B
     const unsigned long long desc0 = tc_smem_desc(0u, slab, 128);
-    // every generator warp set has its own A ring (nab / kTcSets slots): the passes of the items q = kTcSets j + h
-    const unsigned nas = nab / kTcSets, nas_sh = nab_sh - (kTcSets == 2 ? 1u : 0u);
-    unsigned s = 0, ph = 0, n_done = 0;
-    unsigned a_its[kTcSets] = {};
+    unsigned s = 0, ph = 0, a_it = 0, n_done = 0;
     for (int work = blockIdx.x; work < n_work; work += gridDim.x, ++n_done) {
       const int tile_i = work % tp.n_tiles;
       const TcTile td = tp.tiles[tile_i];
@@ -202,32 +201,24 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
         // passes | 16-byte units from the start of the staged window to this group's window << 2
         const unsigned info_l = (unsigned)code_passes(c) |
                                 ((code_passes(c) ? (unsigned)((code_start2(c) >> 1) - wlo) * (slab >> 4) : 0u) << 2);
-        for (int q = 0; q < P.Q; ++q) {
-          const unsigned info = __shfl_sync(0xffffffffu, info_l, q);
-          const int np = (int)(info & 3u);
-          if ((q % kTcIssuers) != par) {                      // the other warp's item: count its ring slots
-            a_its[q % kTcSets] += (unsigned)np;
-          } else {
+        for (int q0 = 0; q0 < P.Q; q0 += kTcQS) {
           mbar_wait_park(b_full0 + 8 * s, ph);                 // also keeps an idle group in step with the ring
-          if (np) {
-            unsigned long long desc = desc0 + (unsigned long long)(((stage0 + s * stage_bytes) >> 4) + (info >> 2));
-            const unsigned set = (unsigned)(q % kTcSets);
-            unsigned a_it = a_its[kTcSets == 2 ? (q & 1) : 0];
+          const int q1 = min(q0 + kTcQS, P.Q);
+          for (int q = q0; q < q1; ++q) {
+            const unsigned info = __shfl_sync(0xffffffffu, info_l, q);
+            const int np = (int)(info & 3u);
+            unsigned long long desc = desc0 + (unsigned long long)(((stage0 + (s * kTcQS + (unsigned)(q - q0)) * stage_bytes) >> 4) + (info >> 2));
             for (int p = 0; p < np; ++p, ++a_it, desc += (unsigned long long)((kTcPassBlocks * slab) >> 4)) {
-              const unsigned buf = set * nas + (a_it & (nas - 1u));
-              mbar_wait_park(af0 + 8u * buf, (a_it >> nas_sh) & 1u);
+              const unsigned buf = a_it & (nab - 1u);
+              mbar_wait_park(af0 + 8u * buf, (a_it >> nab_sh) & 1u);
               tc_fence_after();
               if (tc_elect()) {
                 tc_mma_ts(d_tmem, a_tmem0 + buf * kTcACols, desc, idesc, 1u);
                 tc_commit(ae0 + 8u * buf);                     // A buffer free once this MMA has read it
               }
             }
-            a_its[kTcSets == 2 ? (q & 1) : 0] = a_it;
-            if (tc_elect()) tc_commit(b_empty0 + 8 * s);       // this group is done with the stage
-          } else if (lane == 0) {
-            mbar_arrive(b_empty0 + 8 * s);                     // nothing to read: release at once
           }
-          }
+          if (tc_elect()) tc_commit(b_empty0 + 8 * s);         // this group is done with the stage
           if (++s == (unsigned)tp.n_stages) { s = 0; ph ^= 1u; }
         }
       }

@@ -56,9 +56,8 @@ constexpr int kTcSets = 1;                   // generator warp sets per voxel gr
                                              // per thread with spills and rings of two slots)
 constexpr int kTcQPerSet = 16 / kTcSets;
 constexpr int kTcGenWarps = 4 * kTcSets * kTcG;
-constexpr int kTcIssuers = 1;                // MMA issuer warps per voxel group (2 share the items by the parity of q:
-                                             // correct, measured 109.8 ms against 110.7 ms per 64-frame batch: no gain)
-constexpr int kTcSvcWarps = 1 + kTcIssuers * kTcG;   // TMA producer + the MMA issuers
+constexpr int kTcQS = 4;                     // transmits per stage of the sample ring (one barrier round per kTcQS items)
+constexpr int kTcSvcWarps = 1 + kTcG;        // TMA producer + one MMA issuer per voxel group
 constexpr int kTcThreads = (kTcSvcWarps + kTcGenWarps) * 32;
 constexpr int kTcTmemCols = 512;
 constexpr int kTcACols = 8;                 // TMEM columns of one A buffer (K = 16 FP16 per row)
@@ -76,7 +75,7 @@ struct TcDev {
   int n_tiles, n_chunks;       // work items = n_tiles * n_chunks
   int Bc;                      // frames per chunk; MMA N = 2 Bc
   int KBp;                     // k-blocks per (m, q) row of the converted data, pads included
-  int stage_blocks;            // capacity of one stage in k-blocks
+  int stage_blocks;            // capacity of one window slot in k-blocks (a stage has kTcQS slots)
   int n_stages;                // depth of the stage ring (kTcMinStages..kTcMaxStages)
   int a_bufs, a_shift;         // depth of the A ring per voxel group (2^a_shift <= kTcMaxABufs, what TMEM holds)
   const TcTile* tiles;         // [n_tiles], sorted by decreasing work
@@ -229,7 +228,7 @@ struct alignas(128) TcSmemHeader {
 };
 
 __host__ __device__ inline size_t tc_smem_bytes(int Bc, int stage_blocks, int n_stages) {
-  return sizeof(TcSmemHeader) + 128 + (size_t)n_stages * stage_blocks * (2 * Bc) * 16;
+  return sizeof(TcSmemHeader) + 128 + (size_t)n_stages * kTcQS * stage_blocks * (2 * Bc) * 16;
 }
 
 struct TcPlan;

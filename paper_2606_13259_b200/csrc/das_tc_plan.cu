@@ -213,7 +213,7 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
   if (dv.a_bufs < kTcSets) return refuse_free("tensor memory cannot hold an A ring per generator warp set");
   // The ring only has to cover the L2 latency of a window: measured flat from 4 to 8 stages at the
   // headline, slower at 16 (the CTAs drift apart and L2 holds fewer of their shared windows).
-  dv.n_stages = 6;
+  dv.n_stages = 4;
   if (const char* ev = getenv("DAS_TC_STAGES")) dv.n_stages = std::min(kTcMaxStages, std::max(kTcMinStages, atoi(ev)));   // tuning sweeps only
   while (dv.n_stages > kTcMinStages && tc_smem_bytes(Bc, stage_blocks, dv.n_stages) > 200 * 1024) --dv.n_stages;
   tp->smem = tc_smem_bytes(Bc, stage_blocks, dv.n_stages);
