@@ -10,31 +10,29 @@ namespace {
 
 // Ring state of one generator warp: the A tiles of its voxel group in tensor memory.
 struct TcGenRing {
-  unsigned a_it;        // passes this warp set has written (slot = a_it mod depth, phase = a_it / depth)
+  unsigned a_it;        // passes written so far (slot = a_it mod depth, phase = a_it / depth)
   unsigned pend;        // a_full barrier of the A tile whose store is in flight (a sink while there is none)
-  unsigned nab, nab_sh; // depth of this set's ring and its log2
-  unsigned ae0, af0;    // first a_empty / a_full barrier of this set's ring
-  unsigned a_addr0;     // TMEM address of the ring's slot 0 for this warp's lane quarter
+  unsigned nab, nab_sh; // ring depth and its log2
+  unsigned ae0, af0;    // first a_empty / a_full barrier of the group
+  unsigned a_addr0;     // TMEM address of slot 0 for this warp's lane quarter
   bool lane0;
 };
 
 // One (q, m) item of a generator thread: the two packed weights, the slot of sample k, the passes.
 struct TcItem { unsigned w0, w1; int r, n_pass; };
 
-// The items (q = kTcSets j + h, m) of one receiver for one voxel row.  cw[] holds the 16 window codes of the group
+// The 16 items (q, m) of one receiver for one voxel row.  cw[] holds the 16 window codes of the group
 // (two per word, loaded with one address for the whole warp: no shuffle in the chain).  The item
 // math of q + 1 is written before the stores of q, so that it fills the latency of the
 // store / barrier sequence.  EDGE: the tile's windows touch the ends of the record (reading A6).
 template <bool EDGE>
-__device__ __forceinline__ void tc_gen_receiver(const float (&Tf)[kTcQPerSet], const float (&pc)[kTcQPerSet], const float (&ps)[kTcQPerSet], const int h,
+__device__ __forceinline__ void tc_gen_receiver(const float (&Tf)[16], const float (&pc)[16], const float (&ps)[16],
                                                 const float ex, const float pr, const float pi, const uint4 cw0,
                                                 const uint4 cw1, const int tb_l, const int Q, const int K, TcGenRing& rg) {
   const unsigned cw[8] = {cw0.x, cw0.y, cw0.z, cw0.w, cw1.x, cw1.y, cw1.z, cw1.w};
   auto item = [&](const int j) {
     TcItem it;
-    const int q = kTcSets * j + h;                                   // static when kTcSets == 1
-    const unsigned cww = cw[kTcSets == 2 ? j : (j >> 1)];
-    const unsigned c_q = (q & 1) ? (cww >> 16) : (cww & 0xffffu);
+    const unsigned c_q = (j & 1) ? (cw[j >> 1] >> 16) : (cw[j >> 1] & 0xffffu);
     it.n_pass = code_passes(c_q);
     // fractional index: ki = floor(t) (round-to-nearest of t - 1/2), al = t - ki
     const float t = Tf[j] + ex;
@@ -49,7 +47,7 @@ __device__ __forceinline__ void tc_gen_receiver(const float (&Tf)[kTcQPerSet], c
     it.w1 = pack_half2(w1re, -w1im);
     if (EDGE) {
       // the term is dropped unless 0 <= k <= K-2 (a pad sample may not lend its neighbour a weight)
-      const int tb_q = __shfl_sync(0xffffffffu, tb_l, min(q, Q - 1));
+      const int tb_q = __shfl_sync(0xffffffffu, tb_l, min(j, Q - 1));
       const int ki = (int)(__float_as_uint(u) - kMagicBits);
       if ((unsigned)(ki + tb_q) > (unsigned)(K - 2)) { it.w0 = 0u; it.w1 = 0u; }
     }
@@ -57,9 +55,9 @@ __device__ __forceinline__ void tc_gen_receiver(const float (&Tf)[kTcQPerSet], c
   };
   TcItem cur = item(0);
 #pragma unroll
-  for (int j = 0; j < kTcQPerSet; ++j) {                         // this set's items in transmit order
+  for (int j = 0; j < 16; ++j) {                                 // items in transmit order, q = j
     TcItem nxt = cur;
-    if (j + 1 < kTcQPerSet) nxt = item(j + 1);
+    if (j + 1 < 16) nxt = item(j + 1);
     int r = cur.r;
 #pragma unroll 1
     for (int p = 0; p < cur.n_pass; ++p, r -= kTcBlk * kTcPassBlocks) {
@@ -96,7 +94,8 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
   const unsigned stage0 = (smem_u32(smem_raw) + (unsigned)sizeof(TcSmemHeader) + 127u) & ~127u;
   const int N = 2 * tp.Bc;                                   // MMA N
   const unsigned slab = (unsigned)N * 16u;                   // bytes of one k-block: N columns x 8 FP16
-  const unsigned stage_bytes = (unsigned)tp.stage_blocks * slab;
+  const unsigned stage_bytes = (unsigned)tp.stage_blocks * slab;   // one window slot; a stage has qs of them
+  const unsigned qs = (unsigned)tp.qs;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int n_work = tp.n_tiles * tp.n_chunks;
   const long long n_vox = (long long)P.nx * P.ny * P.nz;
@@ -125,8 +124,8 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
   const unsigned nab = (unsigned)tp.a_bufs, nab_sh = (unsigned)tp.a_shift;   // A ring depth (power of two)
   // The accumulators start from zero and the epilogue leaves them zero again, so every MMA accumulates
   // and no MMA has to be the first of its tile.
-  if (warp < kTcGenWarps && ((warp >> 2) % kTcSets) == 0) {
-    const unsigned d0 = tmem + (((unsigned)((warp & 3) * 32)) << 16) + (unsigned)((warp / (4 * kTcSets)) * N);
+  if (warp < kTcGenWarps) {
+    const unsigned d0 = tmem + (((unsigned)((warp & 3) * 32)) << 16) + (unsigned)((warp >> 2) * N);
     for (int c0 = 0; c0 < N; c0 += 8) tmem_st8_zero(d0 + (unsigned)c0);
     tmem_wait_st();
   }
@@ -136,8 +135,8 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
 
   if (warp == kTcGenWarps) {
     // ===================================== TMA PRODUCER =======================================
-    // A stage holds the windows of kTcQS consecutive transmits of one receiver (one barrier round
-    // per kTcQS items).  Lane q works out the window of item (q, m), the union over the voxel groups,
+    // A stage holds the windows of `qs` consecutive transmits of one receiver (one barrier round
+    // per qs items).  Lane q works out the window of item (q, m), the union over the voxel groups,
     // and issues its own bulk copy; lane 0 waits for the stage and posts the byte count.
     unsigned s = 0, ph = 0;                                  // stage and its phase parity
     const bool has_q = lane < P.Q;
@@ -155,8 +154,8 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
         // byte offset of the window inside the chunk and its length, per lane = q
         const long long src_l = ((long long)hd.x * P.Q * tp.KBp + kTcPadBlocks + (long long)ql * tp.KBp + tb4 + wlo) * (long long)slab;
         const unsigned bytes_l = has_q ? (unsigned)wn * slab : 0u;
-        for (int q0 = 0; q0 < P.Q; q0 += kTcQS) {
-          const bool mine = lane >= q0 && lane < q0 + kTcQS;
+        for (int q0 = 0; q0 < P.Q; q0 += (int)qs) {
+          const bool mine = lane >= q0 && lane < q0 + (int)qs;
           const unsigned total = __reduce_add_sync(0xffffffffu, mine ? bytes_l : 0u);
           if (lane == 0) {
             mbar_wait_park(b_empty0 + 8 * s, ph ^ 1u);
@@ -165,7 +164,7 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
           }
           __syncwarp();
           if (mine && bytes_l)
-            tma_bulk_g2s(stage0 + (s * kTcQS + (unsigned)(lane - q0)) * stage_bytes, base + src_l, bytes_l, b_full0 + 8 * s);
+            tma_bulk_g2s(stage0 + (s * qs + (unsigned)(lane - q0)) * stage_bytes, base + src_l, bytes_l, b_full0 + 8 * s);
           if (++s == (unsigned)tp.n_stages) { s = 0; ph ^= 1u; }
           __syncwarp();
         }
@@ -177,7 +176,7 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
     // latency bounds the MMA rate of a group, so it is kept as short as it can be: lane q prepares
     // item (q, m) (passes, offset of the group's window inside the staged one), every lane runs the
     // same scalar loop (no divergence, one shuffle per item), only the tcgen05 instructions sit
-    // under an elected lane, and the stage barriers are visited once per kTcQS items.
+    // under an elected lane, and the stage barriers are visited once per qs items.
     const int g = warp - kTcGenWarps - 1;
     const unsigned idesc = tc_idesc(N);
     const unsigned d_tmem = tmem + (unsigned)(g * N);
@@ -201,13 +200,13 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
         // passes | 16-byte units from the start of the staged window to this group's window << 2
         const unsigned info_l = (unsigned)code_passes(c) |
                                 ((code_passes(c) ? (unsigned)((code_start2(c) >> 1) - wlo) * (slab >> 4) : 0u) << 2);
-        for (int q0 = 0; q0 < P.Q; q0 += kTcQS) {
+        for (int q0 = 0; q0 < P.Q; q0 += (int)qs) {
           mbar_wait_park(b_full0 + 8 * s, ph);                 // also keeps an idle group in step with the ring
-          const int q1 = min(q0 + kTcQS, P.Q);
+          const int q1 = min(q0 + (int)qs, P.Q);
           for (int q = q0; q < q1; ++q) {
             const unsigned info = __shfl_sync(0xffffffffu, info_l, q);
             const int np = (int)(info & 3u);
-            unsigned long long desc = desc0 + (unsigned long long)(((stage0 + (s * kTcQS + (unsigned)(q - q0)) * stage_bytes) >> 4) + (info >> 2));
+            unsigned long long desc = desc0 + (unsigned long long)(((stage0 + (s * qs + (unsigned)(q - q0)) * stage_bytes) >> 4) + (info >> 2));
             for (int p = 0; p < np; ++p, ++a_it, desc += (unsigned long long)((kTcPassBlocks * slab) >> 4)) {
               const unsigned buf = a_it & (nab - 1u);
               mbar_wait_park(af0 + 8u * buf, (a_it >> nab_sh) & 1u);
@@ -226,8 +225,7 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
     }
   } else {
     // ===================================== GENERATORS =========================================
-    const int g = warp / (4 * kTcSets);                       // voxel group = depth inside the tile
-    const int h = (warp >> 2) % kTcSets;                      // warp set: it takes the transmits q = kTcSets j + h
+    const int g = warp >> 2;                                  // voxel group = depth inside the tile
     const int row = (warp & 3) * 32 + lane;                   // MMA row = TMEM lane (quarter warp % 4)
     const unsigned lane_base = ((unsigned)((warp & 3) * 32)) << 16;
     const unsigned d_addr = tmem + lane_base + (unsigned)(g * N);
@@ -235,12 +233,9 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
     TcGenRing rg;
     rg.a_it = 0;
     rg.pend = smem_u32(&sm.sink);
-    rg.nab = nab / kTcSets; rg.nab_sh = nab_sh - (kTcSets == 2 ? 1u : 0u);
-    rg.ae0 = a_empty0 + 8u * (nab * (unsigned)g + rg.nab * (unsigned)h); rg.af0 = a_full0 + 8u * (nab * (unsigned)g + rg.nab * (unsigned)h);
-    rg.a_addr0 = a_addr0 + rg.nab * (unsigned)h * kTcACols;
-    // epilogue columns of this set: half of D each when a half is a whole number of 16-column loads
-    const bool split = kTcSets == 2 && (N % 32) == 0;
-    const int col_lo = split ? h * (N / 2) : 0, col_hi = split ? col_lo + N / 2 : (h == 0 ? N : 0);
+    rg.nab = nab; rg.nab_sh = nab_sh;
+    rg.ae0 = a_empty0 + 8u * (nab * (unsigned)g); rg.af0 = a_full0 + 8u * (nab * (unsigned)g);
+    rg.a_addr0 = a_addr0;
     rg.lane0 = lane == 0;
     unsigned n_done = 0;
 
@@ -251,10 +246,10 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
       const int tb_l = __ldg(&tp.tbase[(long long)tile_i * P.Q + ql]);
 
       // per-(q, n) part in FP64: reduced transmit delay and transmit phase factor
-      float Tf[kTcQPerSet], pc[kTcQPerSet], ps[kTcQPerSet];
+      float Tf[16], pc[16], ps[16];
 #pragma unroll
-      for (int j = 0; j < kTcQPerSet; ++j) {
-        const int qq = min(kTcSets * j + h, P.Q - 1);
+      for (int j = 0; j < 16; ++j) {
+        const int qq = min(j, P.Q - 1);
         const double T = tc_T(P, vx, qq);
         Tf[j] = (float)(T - (double)__ldg(&tp.tbase[(long long)tile_i * P.Q + qq]));
         double cyc = tp.phase0 + tp.ratio * T;
@@ -293,8 +288,8 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
         cyc -= rintf(cyc);
         const float ang = 6.283185307179586f * cyc;
         const float pr = act ? cos_approx(ang) : 0.f, pi = act ? sin_approx(ang) : 0.f;
-        if (td.edge) tc_gen_receiver<true>(Tf, pc, ps, h, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, rg);
-        else tc_gen_receiver<false>(Tf, pc, ps, h, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, rg);
+        if (td.edge) tc_gen_receiver<true>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, rg);
+        else tc_gen_receiver<false>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, rg);
       }
       tmem_wait_st();
       tc_fence_before();
@@ -306,7 +301,7 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
       tc_fence_after();
       const long long vox = ((long long)vx.ix * P.ny + vx.iy) * P.nz + vx.iz;
       float2* dst = out + (long long)chunk * tp.Bc * n_vox + vox;
-      for (int c0 = col_lo; c0 < col_hi; c0 += 16) {
+      for (int c0 = 0; c0 < N; c0 += 16) {
         float v[16];
         tmem_ld16(d_addr + (unsigned)c0, v);
         tmem_wait_ld();

@@ -51,12 +51,7 @@ constexpr int kTcMaxStages = 16;            // upper bound of the shared-memory 
 constexpr int kTcMinStages = 2;
 constexpr int kTcPadBlocks = 16;            // zero k-blocks before and after every (m, q) row
 constexpr int kTcMaxStageBlocks = 16;       // largest window (k-blocks) one stage can hold
-constexpr int kTcSets = 1;                   // generator warp sets per voxel group (2: even / odd transmits, each with its own
-                                             // A ring; correct, but 119.6 ms against 110.7 ms at the headline: 72 registers
-                                             // per thread with spills and rings of two slots)
-constexpr int kTcQPerSet = 16 / kTcSets;
-constexpr int kTcGenWarps = 4 * kTcSets * kTcG;
-constexpr int kTcQS = 4;                     // transmits per stage of the sample ring (one barrier round per kTcQS items)
+constexpr int kTcGenWarps = 4 * kTcG;
 constexpr int kTcSvcWarps = 1 + kTcG;        // TMA producer + one MMA issuer per voxel group
 constexpr int kTcThreads = (kTcSvcWarps + kTcGenWarps) * 32;
 constexpr int kTcTmemCols = 512;
@@ -75,7 +70,8 @@ struct TcDev {
   int n_tiles, n_chunks;       // work items = n_tiles * n_chunks
   int Bc;                      // frames per chunk; MMA N = 2 Bc
   int KBp;                     // k-blocks per (m, q) row of the converted data, pads included
-  int stage_blocks;            // capacity of one window slot in k-blocks (a stage has kTcQS slots)
+  int stage_blocks;            // capacity of one window slot in k-blocks
+  int qs;                      // window slots (consecutive transmits of one receiver) per stage: one barrier round per qs items
   int n_stages;                // depth of the stage ring (kTcMinStages..kTcMaxStages)
   int a_bufs, a_shift;         // depth of the A ring per voxel group (2^a_shift <= kTcMaxABufs, what TMEM holds)
   const TcTile* tiles;         // [n_tiles], sorted by decreasing work
@@ -227,8 +223,8 @@ struct alignas(128) TcSmemHeader {
   unsigned tmem_base;
 };
 
-__host__ __device__ inline size_t tc_smem_bytes(int Bc, int stage_blocks, int n_stages) {
-  return sizeof(TcSmemHeader) + 128 + (size_t)n_stages * kTcQS * stage_blocks * (2 * Bc) * 16;
+__host__ __device__ inline size_t tc_smem_bytes(int Bc, int stage_blocks, int qs, int n_stages) {
+  return sizeof(TcSmemHeader) + 128 + (size_t)n_stages * qs * stage_blocks * (2 * Bc) * 16;
 }
 
 struct TcPlan;

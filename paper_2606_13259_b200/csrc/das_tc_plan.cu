@@ -210,13 +210,17 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
   if (const char* ev = getenv("DAS_TC_ABUFS")) dv.a_shift = std::min(3, std::max(0, atoi(ev)));   // tuning sweeps only
   while (dv.a_shift > 0 && kTcG * 2 * Bc + kTcG * (1 << dv.a_shift) * kTcACols > kTcTmemCols) --dv.a_shift;
   dv.a_bufs = 1 << dv.a_shift;
-  if (dv.a_bufs < kTcSets) return refuse_free("tensor memory cannot hold an A ring per generator warp set");
-  // The ring only has to cover the L2 latency of a window: measured flat from 4 to 8 stages at the
-  // headline, slower at 16 (the CTAs drift apart and L2 holds fewer of their shared windows).
-  dv.n_stages = 4;
+  // Stage ring: `qs` window slots per stage (the fewer barrier rounds the better: the producer and
+  // the MMA issuers are serial latency chains) and as many stages as cover the L2 latency of a
+  // window.  Measured at the headline: (qs, stages) = (8, 2) 94 ms, (4, 4) 96 ms, (1, 6) 111 ms.
+  dv.qs = 8;
+  dv.n_stages = 2;
+  while (dv.qs > 1 && tc_smem_bytes(Bc, stage_blocks, dv.qs, 2) > 200 * 1024) dv.qs /= 2;
+  if (const char* ev = getenv("DAS_TC_QS")) dv.qs = std::min(16, std::max(1, atoi(ev)));                               // tuning sweeps only
   if (const char* ev = getenv("DAS_TC_STAGES")) dv.n_stages = std::min(kTcMaxStages, std::max(kTcMinStages, atoi(ev)));   // tuning sweeps only
-  while (dv.n_stages > kTcMinStages && tc_smem_bytes(Bc, stage_blocks, dv.n_stages) > 200 * 1024) --dv.n_stages;
-  tp->smem = tc_smem_bytes(Bc, stage_blocks, dv.n_stages);
+  else while (dv.n_stages < 4 && dv.qs * dv.n_stages < 8 && tc_smem_bytes(Bc, stage_blocks, dv.qs, dv.n_stages + 1) <= 200 * 1024) ++dv.n_stages;
+  while (dv.n_stages > kTcMinStages && tc_smem_bytes(Bc, stage_blocks, dv.qs, dv.n_stages) > 200 * 1024) --dv.n_stages;
+  tp->smem = tc_smem_bytes(Bc, stage_blocks, dv.qs, dv.n_stages);
   if (tp->smem > 200 * 1024) return refuse_free("stage ring does not fit in shared memory");
   tp->grid = std::max(1, std::min(n_tiles * dv.n_chunks, prop.multiProcessorCount));
   return tp;
