@@ -145,15 +145,24 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
       const TcTile td = tp.tiles[tile_i];
       const unsigned char* base = convb + (long long)chunk * chunk_bytes;
       const int tb4 = __ldg(&tp.tbase[(long long)tile_i * P.Q + ql]) >> 2;       // k-block of tbase_q
-      for (int li = 0; li < td.list_cnt; ++li) {
-        const long long e = td.list_off + li;
+      // window of item (q = lane, m) of a list entry: byte offset inside the chunk and length; fetched
+      // one entry ahead (the loads are a dependent chain through L2)
+      auto entry_window = [&](const long long e, unsigned& any, unsigned& bytes) {
         const uint2 hd = __ldg(&tp.list[e]);
-        if (!hd.y) continue;
+        any = hd.y;
         int wlo, wn;
         tc_union_window(tp.codes + e * kTcG * 16 + ql, wlo, wn);
-        // byte offset of the window inside the chunk and its length, per lane = q
-        const long long src_l = ((long long)hd.x * P.Q * tp.KBp + kTcPadBlocks + (long long)ql * tp.KBp + tb4 + wlo) * (long long)slab;
-        const unsigned bytes_l = has_q ? (unsigned)wn * slab : 0u;
+        bytes = has_q ? (unsigned)wn * slab : 0u;
+        return ((long long)hd.x * P.Q * tp.KBp + kTcPadBlocks + (long long)ql * tp.KBp + tb4 + wlo) * (long long)slab;
+      };
+      unsigned any_n = 0, bytes_n = 0;
+      long long src_n = 0;
+      if (td.list_cnt) src_n = entry_window(td.list_off, any_n, bytes_n);
+      for (int li = 0; li < td.list_cnt; ++li) {
+        const unsigned any = any_n, bytes_l = bytes_n;
+        const long long src_l = src_n;
+        if (li + 1 < td.list_cnt) src_n = entry_window((long long)td.list_off + li + 1, any_n, bytes_n);
+        if (!any) continue;
         for (int q0 = 0; q0 < P.Q; q0 += (int)qs) {
           const bool mine = lane >= q0 && lane < q0 + (int)qs;
           const unsigned total = __reduce_add_sync(0xffffffffu, mine ? bytes_l : 0u);
@@ -190,16 +199,21 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
       const TcTile td = tp.tiles[tile_i];
       mbar_wait_park(d_empty, (n_done & 1u) ^ 1u);             // epilogue of the previous tile has drained D
       tc_fence_after();
-      for (int li = 0; li < td.list_cnt; ++li) {
-        const long long e = td.list_off + li;
-        const uint2 hd = __ldg(&tp.list[e]);
-        if (!hd.y) continue;
+      // item (q = lane, m) of a list entry: passes | 16-byte units from the start of the staged window to
+      // this group's window << 2; fetched one entry ahead (the loads are a dependent chain through L2)
+      auto entry_info = [&](const long long e, unsigned& any) {
+        any = __ldg(&tp.list[e]).y;
         int wlo, wn;
         tc_union_window(tp.codes + e * kTcG * 16 + ql, wlo, wn);
         const unsigned c = __ldg(&tp.codes[(e * kTcG + g) * 16 + ql]);
-        // passes | 16-byte units from the start of the staged window to this group's window << 2
-        const unsigned info_l = (unsigned)code_passes(c) |
-                                ((code_passes(c) ? (unsigned)((code_start2(c) >> 1) - wlo) * (slab >> 4) : 0u) << 2);
+        return (unsigned)code_passes(c) | ((code_passes(c) ? (unsigned)((code_start2(c) >> 1) - wlo) * (slab >> 4) : 0u) << 2);
+      };
+      unsigned any_n = 0, info_n = 0;
+      if (td.list_cnt) info_n = entry_info(td.list_off, any_n);
+      for (int li = 0; li < td.list_cnt; ++li) {
+        const unsigned any = any_n, info_l = info_n;
+        if (li + 1 < td.list_cnt) info_n = entry_info((long long)td.list_off + li + 1, any_n);
+        if (!any) continue;
         for (int q0 = 0; q0 < P.Q; q0 += (int)qs) {
           mbar_wait_park(b_full0 + 8 * s, ph);                 // also keeps an idle group in step with the ring
           const int q1 = min(q0 + (int)qs, P.Q);
