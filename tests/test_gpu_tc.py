@@ -170,6 +170,31 @@ def test_tc_headline_full_size_batch64_sampled(das_lib):
         assert emax <= TOL_FP16_MAX and el2 <= TOL_FP16_L2, f"slot {b}: max {emax:.3e}, L2 {el2:.3e}"
 
 
+def test_tc_headline_geometry_reduced_grid_full(das_lib):
+    """Headline array, 16 diverging-wave transmits and native voxel spacing on a 40 x 24 x 9 block of
+    the grid (several tiles, ragged in every axis), every voxel compared: the 8-transmits-per-stage
+    sample ring and the 16-transmit generator loop at full width."""
+    w = _subgrid(3, slice(30, 70), slice(50, 74), slice(60, 69))
+    yb = make_batch(w.y, 8, 110)
+    got = gpu_batch(das_lib, w, yb)
+    check_frames(got, w, yb, frames=[0, 5], label="config3 sub-grid B=8")
+
+
+def test_tc_headline_geometry_record_edges(das_lib):
+    """The same with a record cut so short that the deep voxels run off its end and t_start moved so
+    that the shallow ones start before sample 0: the per-tile edge path (reading A6) with 16 transmits."""
+    import oracle
+    base = _subgrid(3, slice(56, 72), slice(60, 68), slice(0, 128, 5))
+    y = np.ascontiguousarray(base.y[:, :, 60:260])
+    w = wl.custom(base.elem_pos, base.tx_type, base.tx_v, base.tx_t0, base.xs, base.ys, base.zs,
+                  fs=base.fs, n_samples=200, t_start=60.0 / base.fs, f_number=1.0, y=y)
+    cnt = oracle.das(w, want_count=True)["count"]
+    assert cnt.min() < cnt.max() and (cnt == 0).any()
+    yb = make_batch(y, 8, 111)
+    got = gpu_batch(das_lib, w, yb)
+    check_frames(got, w, yb, frames=[0, 7], label="config3 record edges")
+
+
 # ------------------------------------------------------------------ dispatch rules
 
 def test_tc_refusals_and_fallback(das_lib):
