@@ -172,6 +172,10 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
       (e = cudaMemcpy(edge.data(), d_edge, sizeof(int) * n_tiles, cudaMemcpyDeviceToHost)) != cudaSuccess ||
       (e = cudaMemcpy(stats, d_stats, sizeof(stats), cudaMemcpyDeviceToHost)) != cudaSuccess) return fail(e);
   auto refuse_free = [&](const char* msg) -> TcPlan* { tc_plan_destroy(tp); return refuse(msg); };
+  if (getenv("DAS_TC_VERBOSE")) {
+    long long tw = 0; for (int w_ : work) tw += w_;
+    fprintf(stderr, "[das tc plan] tiles %d, list entries %zu, MMA passes %lld, largest window %d k-blocks\n", n_tiles, list.size(), tw, stats[0]);
+  }
   if (stats[1] & 1) return refuse_free("a sample window of a voxel group needs more than 3 MMA passes (grid too coarse)");
   if (stats[1] & 2) return refuse_free("a sample window leaves the zero-padded record");
   if (stats[1] & 4) return refuse_free("internal: negative window start");
