@@ -22,42 +22,48 @@ struct TcGenRing {
 struct TcItem { unsigned w0, w1; int r, n_pass; };
 
 // The 16 items (q, m) of one receiver for one voxel row.  cw[] holds the 16 window codes of the group
-// (two per word, loaded with one address for the whole warp: no shuffle in the chain).  The item
-// math of q + 1 is written before the stores of q, so that it fills the latency of the
-// store / barrier sequence.  EDGE: the tile's windows touch the ends of the record (reading A6).
+// (two per word, loaded with one address for the whole warp: no shuffle in the chain).  The index and
+// weight arithmetic runs on transmit PAIRS as packed FP32x2 instructions (FADD2 / FMUL2 / FFMA2, sm_100),
+// and the pair after the current one is worked out before the stores of the current one, so that it
+// fills the latency of the store / barrier sequence.  EDGE: the tile's windows touch the ends of the
+// record (reading A6).  Tf2 / pc2 / ps2: (q = 2 j, q = 2 j + 1).
 template <bool EDGE>
-__device__ __forceinline__ void tc_gen_receiver(const float (&Tf)[16], const float (&pc)[16], const float (&ps)[16],
+__device__ __forceinline__ void tc_gen_receiver(const float2 (&Tf2)[8], const float2 (&pc2)[8], const float2 (&ps2)[8],
                                                 const float ex, const float pr, const float pi, const uint4 cw0,
                                                 const uint4 cw1, const int tb_l, const int Q, const int K, TcGenRing& rg) {
   const unsigned cw[8] = {cw0.x, cw0.y, cw0.z, cw0.w, cw1.x, cw1.y, cw1.z, cw1.w};
-  auto item = [&](const int j) {
-    TcItem it;
-    const unsigned c_q = (j & 1) ? (cw[j >> 1] >> 16) : (cw[j >> 1] & 0xffffu);
-    it.n_pass = code_passes(c_q);
+  const float2 ex2 = make_float2(ex, ex), pr2 = make_float2(pr, pr), npr2 = make_float2(-pr, -pr);
+  const float2 npi2 = make_float2(-pi, -pi);
+  const float2 mh2 = make_float2(-0.5f, -0.5f), mg2 = make_float2(kMagic, kMagic), nmg2 = make_float2(-kMagic, -kMagic);
+  auto item_pair = [&](const int jp, TcItem& i0, TcItem& i1) {
+    const unsigned c0 = cw[jp] & 0xffffu, c1 = cw[jp] >> 16;
+    i0.n_pass = code_passes(c0);
+    i1.n_pass = code_passes(c1);
     // fractional index: ki = floor(t) (round-to-nearest of t - 1/2), al = t - ki
-    const float t = Tf[j] + ex;
-    const float u = (t - 0.5f) + kMagic;
-    const float al = t - (u - kMagic);
+    const float2 t = __fadd2_rn(Tf2[jp], ex2);
+    const float2 u = __fadd2_rn(__fadd2_rn(t, mh2), mg2);
+    const float2 al = __ffma2_rn(__fadd2_rn(u, nmg2), make_float2(-1.f, -1.f), t);
     // slot of sample k inside the item's window:  r = ki - window start
-    it.r = (int)__float_as_uint(u) - (int)(kMagicBits + 2u * (unsigned)code_start2(c_q));
-    // weights: P = Ptx_q Prx_m;  W1 = al P (sample k + 1),  W0 = P - W1 (sample k)
-    const float wre = fmaf(pc[j], pr, -ps[j] * pi), wim = fmaf(pc[j], pi, ps[j] * pr);
-    const float w1re = al * wre, w1im = al * wim;
-    it.w0 = pack_half2(wre - w1re, w1im - wim);                    // (Re W0, -Im W0)
-    it.w1 = pack_half2(w1re, -w1im);
+    i0.r = (int)__float_as_uint(u.x) - (int)(kMagicBits + 2u * (unsigned)code_start2(c0));
+    i1.r = (int)__float_as_uint(u.y) - (int)(kMagicBits + 2u * (unsigned)code_start2(c1));
+    // weights: P = Ptx_q Prx_m;  W1 = al P (sample k + 1),  W0 = P - W1 (sample k); the imaginary parts
+    // are carried negated (the A row holds (Re W, -Im W))
+    const float2 wre = __ffma2_rn(pc2[jp], pr2, __fmul2_rn(ps2[jp], npi2));          //  Re P
+    const float2 nwim = __ffma2_rn(pc2[jp], npi2, __fmul2_rn(ps2[jp], npr2));        // -Im P
+    const float2 w1re = __fmul2_rn(al, wre), nw1im = __fmul2_rn(al, nwim);
+    const float2 w0re = __ffma2_rn(w1re, make_float2(-1.f, -1.f), wre);
+    const float2 nw0im = __ffma2_rn(nw1im, make_float2(-1.f, -1.f), nwim);
+    i0.w0 = pack_half2(w0re.x, nw0im.x); i0.w1 = pack_half2(w1re.x, nw1im.x);
+    i1.w0 = pack_half2(w0re.y, nw0im.y); i1.w1 = pack_half2(w1re.y, nw1im.y);
     if (EDGE) {
       // the term is dropped unless 0 <= k <= K-2 (a pad sample may not lend its neighbour a weight)
-      const int tb_q = __shfl_sync(0xffffffffu, tb_l, min(j, Q - 1));
-      const int ki = (int)(__float_as_uint(u) - kMagicBits);
-      if ((unsigned)(ki + tb_q) > (unsigned)(K - 2)) { it.w0 = 0u; it.w1 = 0u; }
+      const int tb0 = __shfl_sync(0xffffffffu, tb_l, min(2 * jp, Q - 1)), tb1 = __shfl_sync(0xffffffffu, tb_l, min(2 * jp + 1, Q - 1));
+      const int k0 = (int)(__float_as_uint(u.x) - kMagicBits), k1 = (int)(__float_as_uint(u.y) - kMagicBits);
+      if ((unsigned)(k0 + tb0) > (unsigned)(K - 2)) { i0.w0 = 0u; i0.w1 = 0u; }
+      if ((unsigned)(k1 + tb1) > (unsigned)(K - 2)) { i1.w0 = 0u; i1.w1 = 0u; }
     }
-    return it;
   };
-  TcItem cur = item(0);
-#pragma unroll
-  for (int j = 0; j < 16; ++j) {                                 // items in transmit order, q = j
-    TcItem nxt = cur;
-    if (j + 1 < 16) nxt = item(j + 1);
+  auto passes = [&](const TcItem& cur) {
     int r = cur.r;
 #pragma unroll 1
     for (int p = 0; p < cur.n_pass; ++p, r -= kTcBlk * kTcPassBlocks) {
@@ -82,7 +88,16 @@ __device__ __forceinline__ void tc_gen_receiver(const float (&Tf)[16], const flo
       rg.pend = rg.af0 + 8u * buf;
       ++rg.a_it;
     }
-    cur = nxt;
+  };
+  TcItem c0, c1;
+  item_pair(0, c0, c1);
+#pragma unroll
+  for (int jp = 0; jp < 8; ++jp) {                               // items in transmit order, q = 2 jp, 2 jp + 1
+    TcItem n0 = c0, n1 = c1;
+    if (jp + 1 < 8) item_pair(jp + 1, n0, n1);
+    passes(c0);
+    passes(c1);
+    c0 = n0; c1 = n1;
   }
 }
 
@@ -260,17 +275,17 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
       const int tb_l = __ldg(&tp.tbase[(long long)tile_i * P.Q + ql]);
 
       // per-(q, n) part in FP64: reduced transmit delay and transmit phase factor
-      float Tf[16], pc[16], ps[16];
+      float2 Tf[8], pc[8], ps[8];                               // (q = 2 j, q = 2 j + 1)
 #pragma unroll
       for (int j = 0; j < 16; ++j) {
         const int qq = min(j, P.Q - 1);
         const double T = tc_T(P, vx, qq);
-        Tf[j] = (float)(T - (double)__ldg(&tp.tbase[(long long)tile_i * P.Q + qq]));
+        const float tf = (float)(T - (double)__ldg(&tp.tbase[(long long)tile_i * P.Q + qq]));
         double cyc = tp.phase0 + tp.ratio * T;
         cyc -= rint(cyc);
         const float ang = 6.283185307179586f * (float)cyc;
-        pc[j] = cos_approx(ang);
-        ps[j] = sin_approx(ang);
+        if (j & 1) { Tf[j >> 1].y = tf; pc[j >> 1].y = cos_approx(ang); ps[j >> 1].y = sin_approx(ang); }
+        else       { Tf[j >> 1].x = tf; pc[j >> 1].x = cos_approx(ang); ps[j >> 1].x = sin_approx(ang); }
       }
 
       // the list entry one iteration ahead: header, the group's 16 window codes, receiver position
