@@ -63,7 +63,7 @@ N_SM = 148
 # `ncu --set full` capture summarised in profiles/ (bytes); keyed by (config, storage).
 NCU_TRAFFIC_BYTES = {
     (3, "fp16", 1): 57.05e6,     # profiles/r1_tiled_v3_iq16_full.md
-    (3, "fp16", 64): 176.2e9,    # profiles/r1_tc_b64_full.md
+    (3, "fp16", 64): 175.3e9,    # profiles/r1_tc_b64_full.md
 }
 
 
@@ -433,7 +433,7 @@ def run_cuda(args):
         bound = "tensor"
         flops_model = (f"{FLOPS_PER_TERM[w.data_kind]:.0f} x entered terms x {B} frames + {FLOPS_PER_PAIR:.0f} x active (m,n) pairs "
                        f"(DESIGN.md); the MMAs the kernel issues carry 4x to 5x as many (2 of 8 samples of a K = 16 pass are non-zero)")
-        extra = {"ncu": {"tensor_pipe_active": 0.43, "issue_slots_active": 0.67, "alu_pipe_active": 0.61,
+        extra = {"ncu": {"tensor_pipe_active": 0.44, "issue_slots_active": 0.64, "alu_pipe_active": 0.62,
                          "source": "profiles/r1_tc_b64_full.md"}}
     achieved = flops / (exec_ms * 1e-3) / 1e12
     traffic = NCU_TRAFFIC_BYTES.get((args.config, args.storage, B)) if algo_used != "general" else None
