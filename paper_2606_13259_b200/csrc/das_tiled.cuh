@@ -42,7 +42,7 @@ namespace das {
 
 constexpr int kRawStages = 4;                   // ring of TMA-staged windows (storage precision)
 constexpr int kTabStages = 4;                   // ring of FP32 line tables the consumers read
-constexpr int kConvWarps = 2;
+constexpr int kConvWarps = 3;
 constexpr int kHelperWarps = 4;                 // one warpgroup: producer + converters (+ idle)
 constexpr int kLaneX = 8, kLaneY = 4;          // a consumer warp covers 8 x 4 lateral voxels
 constexpr int kWX = 1, kWY = 2, kWZ = 4;       // consumer warps per tile: tile = 8 x 8 x 4 voxels
