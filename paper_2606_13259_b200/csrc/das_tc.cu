@@ -2,35 +2,161 @@
 #include <climits>
 #include <cstdlib>
 
+#include <cuda.h>
+
 #include "das_tc.cuh"
 
 namespace das {
 
 namespace {
 
-// Ring state of one generator warp: the A tiles of its voxel group in tensor memory.
-struct TcGenRing {
-  unsigned a_it;        // passes written so far (slot = a_it mod depth, phase = a_it / depth)
-  unsigned pend;        // a_full barrier of the A tile whose store is in flight (a sink while there is none)
-  unsigned nab, nab_sh; // ring depth and its log2
-  unsigned ae0, af0;    // first a_empty / a_full barrier of the group
+// Cycle accounting of the barrier waits per warp role (compile with -DDAS_TC_PROF, run with DAS_TC_PROF=1):
+// prof[cta][warp][k]: k = 0 total cycles of the role loop, 1..6 cycles spent in the waits listed at the use sites.
+#ifdef DAS_TC_PROF
+#define TC_PROF_DECL unsigned long long pf_[8] = {0, 0, 0, 0, 0, 0, 0, 0}; const long long pf_t0_ = clock64();
+#define TC_PROF_WAIT(k, stmt) { const long long c0_ = clock64(); stmt; pf_[k] += (unsigned long long)(clock64() - c0_); }
+#define TC_PROF_END if (tp.prof && lane == 0) { pf_[0] = (unsigned long long)(clock64() - pf_t0_); for (int k_ = 0; k_ < 8; ++k_) tp.prof[((long long)blockIdx.x * 32 + warp) * 8 + k_] = pf_[k_]; }
+#else
+#define TC_PROF_DECL
+#define TC_PROF_WAIT(k, stmt) { stmt; }
+#define TC_PROF_END
+#endif
+
+// State of one generator warp: the A slots of its voxel group in tensor memory (das_tc.cuh).
+struct TcGenState {
   unsigned a_addr0;     // TMEM address of slot 0 for this warp's lane quarter
+  unsigned af0, ae0;    // a_full / a_empty barrier of slot 0 of the group (shared-memory addresses)
+  unsigned pend;        // a_full barrier of the item tile whose store is in flight (the sink while there is none)
+  unsigned sink;
+  unsigned par;         // bit s: phase parity of the next use of slot s (bit kTcOvf: the overflow slot)
+  unsigned it;          // item tiles stored so far (slot = it mod 4 when the transmit count is not 16)
+#ifdef DAS_TC_PROF
+  unsigned long long pf1, pf2, pf3;
+#endif
+  bool free_next;       // the next item's slot was seen free by the probe issued one item ahead
+  bool ovf_pend;        // an overflow tile's store is in flight
   bool lane0;
 };
 
 // One (q, m) item of a generator thread: the two packed weights, the slot of sample k, the passes.
 struct TcItem { unsigned w0, w1; int r, n_pass; };
 
+// The A row of one MMA pass: slot r holds W0, slot r + 1 holds W1, every other slot 0 (r in [-1, 7]).
+__device__ __forceinline__ void tc_place(const int r, const unsigned w0, const unsigned w1, unsigned (&v)[8]) {
+#pragma unroll
+  for (int i = 0; i < 8; ++i) v[i] = 0u;
+#pragma unroll
+  for (int i = -1; i < 8; ++i) {                               // 9 compares, 16 selects
+    const bool hit = r == i;
+    if (i >= 0) v[i] = hit ? w0 : v[i];
+    if (i < 7) v[i + 1] = hit ? w1 : v[i + 1];
+  }
+}
+
+// One NON-BLOCKING probe of an mbarrier phase (test_wait: a scoreboarded read, unlike try_wait, which
+// suspends the warp for 60-150 cycles even when the phase has long completed).  The result is consumed
+// an item later, so the probe's latency overlaps the placement arithmetic.
+__device__ __forceinline__ bool mbar_test(unsigned bar, unsigned parity) {
+  unsigned ok;
+  asm volatile("{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+               : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ unsigned lds_volatile(unsigned addr) {
+  unsigned v;
+  asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+  return v;
+}
+// mbarrier arrive under a predicate (no branch: the warp stays converged for the .sync.aligned tcgen05 ops)
+__device__ __forceinline__ void mbar_arrive_if(unsigned bar, bool pred) {
+  asm volatile("{\n\t.reg .pred p;\n\t.reg .b64 st;\n\tsetp.ne.b32 p, %1, 0;\n\t@p mbarrier.arrive.shared::cta.b64 st, [%0];\n\t}"
+               ::"r"(bar), "r"((unsigned)pred) : "memory");
+}
+
+// Third pass of an item (rare: very wide windows), kept out of line.  The overflow tile of the second pass
+// has to be consumed first, and the issuer takes the item tile before it: both stores are completed here,
+// then the overflow slot is reused.  Returns the updated parity word; the caller resets `pend`.
+static __device__ __noinline__ unsigned tc_third_pass(int r, unsigned w0, unsigned w1, unsigned pend, unsigned af0, unsigned ae0,
+                                                      unsigned a_addr0, unsigned par, bool lane0) {
+  unsigned v[8];
+  tc_place(r, w0, w1, v);                                     // r = 8: an all-zero row
+  tmem_wait_st();
+  tc_fence_before();
+  mbar_arrive_if(pend, lane0);
+  mbar_arrive_if(af0 + 8u * kTcOvf, lane0);
+  mbar_wait_park(ae0 + 8u * kTcOvf, ((par >> kTcOvf) & 1u) ^ 1u);
+  tc_fence_after();
+  tmem_st8(a_addr0 + kTcOvf * kTcACols, v);
+  return par ^ (1u << kTcOvf);
+}
+
+// Hand item I of the current receiver to the MMA issuer.  With 16 transmits per receiver (Q16) the slot
+// S = I mod 4 and the barrier phases are compile-time constants.  Order of events:
+//   placement of this item | completion of the PREVIOUS item's stores (they have had the placement to land)
+//   | slot S free? (probed one item ahead) | store | probe of the next item's slot | overflow pass.
+template <bool ZERO, bool Q16, int I>
+__device__ __forceinline__ void tc_gen_item(const TcItem& cur, TcGenState& st) {
+  const unsigned S = Q16 ? (unsigned)(I & (kTcSlots - 1)) : (st.it & (unsigned)(kTcSlots - 1));
+  const unsigned pe = Q16 ? (unsigned)(((I / kTcSlots) & 1) ^ 1) : (((st.par >> S) & 1u) ^ 1u);
+  bool ovf_free = false;
+  if (cur.n_pass > 1) ovf_free = mbar_test(st.ae0 + 8u * kTcOvf, ((st.par >> kTcOvf) & 1u) ^ 1u);
+  unsigned v[8];
+  if (!ZERO) tc_place(cur.r, cur.w0, cur.w1, v);
+#ifdef DAS_TC_PROF
+  { const long long c0_ = clock64(); tmem_wait_st(); st.pf3 += (unsigned long long)(clock64() - c0_); }
+#else
+  tmem_wait_st();
+#endif
+  tc_fence_before();
+  mbar_arrive_if(st.pend, st.lane0);
+  mbar_arrive_if(st.af0 + 8u * kTcOvf, st.lane0 && st.ovf_pend);
+  st.ovf_pend = false;
+#ifdef DAS_TC_PROF
+  if (!st.free_next) { const long long c0_ = clock64(); mbar_wait_park(st.ae0 + 8u * S, pe); st.pf1 += (unsigned long long)(clock64() - c0_); }
+#else
+  if (!st.free_next) mbar_wait_park(st.ae0 + 8u * S, pe);
+#endif
+  tc_fence_after();
+  if (ZERO) tmem_st8_zero(st.a_addr0 + S * kTcACols); else tmem_st8(st.a_addr0 + S * kTcACols, v);
+  st.pend = st.af0 + 8u * S;
+  if (!Q16) { st.par ^= 1u << S; ++st.it; }
+  {
+    // probe the slot of the next item (of this receiver or of the next one)
+    const unsigned Sn = Q16 ? (unsigned)((I + 1) & (kTcSlots - 1)) : (st.it & (unsigned)(kTcSlots - 1));
+    const unsigned pn = Q16 ? (unsigned)(((((I + 1) & 15) / kTcSlots) & 1) ^ 1) : (((st.par >> Sn) & 1u) ^ 1u);
+    st.free_next = mbar_test(st.ae0 + 8u * Sn, pn);
+  }
+  if (cur.n_pass > 1) {
+    // the second pass of the window goes through the overflow slot (uniform branch, ~30 % of the items)
+    if (!ZERO) tc_place(cur.r - kTcBlk * kTcPassBlocks, cur.w0, cur.w1, v);
+#ifdef DAS_TC_PROF
+    if (!ovf_free) { const long long c0_ = clock64(); mbar_wait_park(st.ae0 + 8u * kTcOvf, ((st.par >> kTcOvf) & 1u) ^ 1u); st.pf2 += (unsigned long long)(clock64() - c0_); }
+#else
+    if (!ovf_free) mbar_wait_park(st.ae0 + 8u * kTcOvf, ((st.par >> kTcOvf) & 1u) ^ 1u);
+#endif
+    st.par ^= 1u << kTcOvf;
+    tc_fence_after();
+    if (ZERO) tmem_st8_zero(st.a_addr0 + kTcOvf * kTcACols); else tmem_st8(st.a_addr0 + kTcOvf * kTcACols, v);
+    if (cur.n_pass > 2) {
+      st.par = tc_third_pass(ZERO ? 8 : cur.r - 2 * kTcBlk * kTcPassBlocks, cur.w0, cur.w1, st.pend, st.af0, st.ae0, st.a_addr0, st.par, st.lane0);
+      st.pend = st.sink;
+    }
+    st.ovf_pend = true;
+  }
+}
+
 // The 16 items (q, m) of one receiver for one voxel row.  cw[] holds the 16 window codes of the group
 // (two per word, loaded with one address for the whole warp: no shuffle in the chain).  The index and
 // weight arithmetic runs on transmit PAIRS as packed FP32x2 instructions (FADD2 / FMUL2 / FFMA2, sm_100),
 // and the pair after the current one is worked out before the stores of the current one, so that it
 // fills the latency of the store / barrier sequence.  EDGE: the tile's windows touch the ends of the
-// record (reading A6).  Tf2 / pc2 / ps2: (q = 2 j, q = 2 j + 1).
-template <bool EDGE>
+// record (reading A6).  ZERO: no voxel of this warp sees the receiver (all rows are zero: only the
+// slot protocol runs).  Q16: 16 transmits, every slot is used 4 times per receiver, so the barrier
+// phases are compile-time constants.  Tf2 / pc2 / ps2: (q = 2 j, q = 2 j + 1).
+template <bool EDGE, bool ZERO, bool Q16>
 __device__ __forceinline__ void tc_gen_receiver(const float2 (&Tf2)[8], const float2 (&pc2)[8], const float2 (&ps2)[8],
                                                 const float ex, const float pr, const float pi, const uint4 cw0,
-                                                const uint4 cw1, const int tb_l, const int Q, const int K, TcGenRing& rg) {
+                                                const uint4 cw1, const int tb_l, const int Q, const int K, TcGenState& st) {
   const unsigned cw[8] = {cw0.x, cw0.y, cw0.z, cw0.w, cw1.x, cw1.y, cw1.z, cw1.w};
   const float2 ex2 = make_float2(ex, ex), pr2 = make_float2(pr, pr), npr2 = make_float2(-pr, -pr);
   const float2 npi2 = make_float2(-pi, -pi);
@@ -39,13 +165,14 @@ __device__ __forceinline__ void tc_gen_receiver(const float2 (&Tf2)[8], const fl
     const unsigned c0 = cw[jp] & 0xffffu, c1 = cw[jp] >> 16;
     i0.n_pass = code_passes(c0);
     i1.n_pass = code_passes(c1);
+    if (ZERO) return;
     // fractional index: ki = floor(t) (round-to-nearest of t - 1/2), al = t - ki
     const float2 t = __fadd2_rn(Tf2[jp], ex2);
     const float2 u = __fadd2_rn(__fadd2_rn(t, mh2), mg2);
     const float2 al = __ffma2_rn(__fadd2_rn(u, nmg2), make_float2(-1.f, -1.f), t);
     // slot of sample k inside the item's window:  r = ki - window start
-    i0.r = (int)__float_as_uint(u.x) - (int)(kMagicBits + 2u * (unsigned)code_start2(c0));
-    i1.r = (int)__float_as_uint(u.y) - (int)(kMagicBits + 2u * (unsigned)code_start2(c1));
+    i0.r = (int)__float_as_uint(u.x) - (int)(kMagicBits + (unsigned)code_start(c0));
+    i1.r = (int)__float_as_uint(u.y) - (int)(kMagicBits + (unsigned)code_start(c1));
     // weights: P = Ptx_q Prx_m;  W1 = al P (sample k + 1),  W0 = P - W1 (sample k); the imaginary parts
     // are carried negated (the A row holds (Re W, -Im W))
     const float2 wre = __ffma2_rn(pc2[jp], pr2, __fmul2_rn(ps2[jp], npi2));          //  Re P
@@ -63,70 +190,56 @@ __device__ __forceinline__ void tc_gen_receiver(const float2 (&Tf2)[8], const fl
       if ((unsigned)(k1 + tb1) > (unsigned)(K - 2)) { i1.w0 = 0u; i1.w1 = 0u; }
     }
   };
-  auto passes = [&](const TcItem& cur) {
-    int r = cur.r;
-#pragma unroll 1
-    for (int p = 0; p < cur.n_pass; ++p, r -= kTcBlk * kTcPassBlocks) {
-      // the A row of this MMA: slot r holds W0, slot r + 1 holds W1, every other slot 0
-      unsigned v[8];
-#pragma unroll
-      for (int i = 0; i < 8; ++i) v[i] = 0u;
-#pragma unroll
-      for (int i = -1; i < 8; ++i) {
-        const bool hit = r == i;
-        if (i >= 0) v[i] = hit ? cur.w0 : v[i];
-        if (i < 7) v[i + 1] = hit ? cur.w1 : v[i + 1];
-      }
-      const unsigned buf = rg.a_it & (rg.nab - 1u);
-      // complete the previous A tile (its store has had the placement above to land)
-      tmem_wait_st();
-      tc_fence_before();
-      if (rg.lane0) mbar_arrive(rg.pend);
-      mbar_wait_park(rg.ae0 + 8u * buf, ((rg.a_it >> rg.nab_sh) & 1u) ^ 1u);
-      tc_fence_after();
-      tmem_st8(rg.a_addr0 + buf * kTcACols, v);
-      rg.pend = rg.af0 + 8u * buf;
-      ++rg.a_it;
-    }
-  };
   TcItem c0, c1;
+  c0.w0 = c0.w1 = c1.w0 = c1.w1 = 0u; c0.r = c1.r = 0;
   item_pair(0, c0, c1);
-#pragma unroll
-  for (int jp = 0; jp < 8; ++jp) {                               // items in transmit order, q = 2 jp, 2 jp + 1
-    TcItem n0 = c0, n1 = c1;
-    if (jp + 1 < 8) item_pair(jp + 1, n0, n1);
-    passes(c0);
-    passes(c1);
-    c0 = n0; c1 = n1;
+#define DAS_TC_PAIR(JP)                                                        \
+  {                                                                            \
+    TcItem n0 = c0, n1 = c1;                                                   \
+    if (JP + 1 < 8) item_pair(JP + 1, n0, n1);                                 \
+    if (Q16 || c0.n_pass) tc_gen_item<ZERO, Q16, 2 * JP>(c0, st);              \
+    if (Q16 || c1.n_pass) tc_gen_item<ZERO, Q16, 2 * JP + 1>(c1, st);          \
+    c0 = n0; c1 = n1;                                                          \
   }
+  DAS_TC_PAIR(0) DAS_TC_PAIR(1) DAS_TC_PAIR(2) DAS_TC_PAIR(3)
+  DAS_TC_PAIR(4) DAS_TC_PAIR(5) DAS_TC_PAIR(6) DAS_TC_PAIR(7)
+#undef DAS_TC_PAIR
 }
 
 // Work items: (chunk, tile), tile fastest; every warp role walks the same sequence.
 __global__ void __launch_bounds__(kTcThreads, 1)
-tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ convb, float2* __restrict__ out) {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
+tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tmap_small,
+          const __grid_constant__ CUtensorMap tmap_big, float2* __restrict__ out) {
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
   TcSmemHeader& sm = *reinterpret_cast<TcSmemHeader*>(smem_raw);
-  const unsigned stage0 = (smem_u32(smem_raw) + (unsigned)sizeof(TcSmemHeader) + 127u) & ~127u;
+  const unsigned stage0 = (smem_u32(smem_raw) + (unsigned)sizeof(TcSmemHeader) + 1023u) & ~1023u;
   const int N = 2 * tp.Bc;                                   // MMA N
-  const unsigned slab = (unsigned)N * 16u;                   // bytes of one k-block: N columns x 8 FP16
-  const unsigned stage_bytes = (unsigned)tp.stage_blocks * slab;   // one window slot; a stage has qs of them
+  const unsigned stage_bytes = tc_box_bytes(tp.Bc, kTcBoxBig);    // one window slot holds one box; a stage has qs of them
+  const unsigned small_bytes = tc_box_bytes(tp.Bc, kTcBoxSmall);
   const unsigned qs = (unsigned)tp.qs;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int n_work = tp.n_tiles * tp.n_chunks;
   const long long n_vox = (long long)P.nx * P.ny * P.nz;
-  const long long chunk_bytes = (long long)P.M * P.Q * tp.KBp * slab;
   const int ql = min(lane & 15, P.Q - 1);                    // the transmit this lane reads windows for
+  const bool q16 = P.Q == 16;
 
-  const unsigned b_full0 = smem_u32(&sm.b_full[0]), b_empty0 = smem_u32(&sm.b_empty[0]);
-  const unsigned a_full0 = smem_u32(&sm.a_full[0]), a_empty0 = smem_u32(&sm.a_empty[0]);
-  const unsigned d_full = smem_u32(&sm.d_full), d_empty = smem_u32(&sm.d_empty);
+  // barrier addresses: taken once through an opaque move so that ptxas keeps them in registers instead of
+  // rebuilding the shared-window base (S2UR + ULEA) at every use
+  unsigned b_full0, b_empty0, a_full0, a_empty0, d_full, d_empty, sinkb;
+  asm volatile("mov.u32 %0, %1;" : "=r"(b_full0) : "r"(smem_u32(&sm.b_full[0])));
+  asm volatile("mov.u32 %0, %1;" : "=r"(b_empty0) : "r"(smem_u32(&sm.b_empty[0])));
+  asm volatile("mov.u32 %0, %1;" : "=r"(a_full0) : "r"(smem_u32(&sm.a_full[0])));
+  asm volatile("mov.u32 %0, %1;" : "=r"(a_empty0) : "r"(smem_u32(&sm.a_empty[0])));
+  asm volatile("mov.u32 %0, %1;" : "=r"(d_full) : "r"(smem_u32(&sm.d_full)));
+  asm volatile("mov.u32 %0, %1;" : "=r"(d_empty) : "r"(smem_u32(&sm.d_empty)));
+  asm volatile("mov.u32 %0, %1;" : "=r"(sinkb) : "r"(smem_u32(&sm.sink)));
 
   if (tid == 0) {
-    for (int s = 0; s < kTcMaxStages; ++s) { mbar_init(b_full0 + 8 * s, 1); mbar_init(b_empty0 + 8 * s, kTcG); }
-    for (int i = 0; i < kTcMaxABufs * kTcG; ++i) { mbar_init(a_full0 + 8 * i, 4); mbar_init(a_empty0 + 8 * i, 1); }
-    mbar_init(d_full, kTcG);
+    for (int s = 0; s < kTcMaxStages; ++s) { mbar_init(b_full0 + 8 * s, 1); mbar_init(b_empty0 + 8 * s, kTcG * kTcIss); }
+    for (int i = 0; i < kTcABufs * kTcG; ++i) { mbar_init(a_full0 + 8 * i, 4); mbar_init(a_empty0 + 8 * i, 1); }
+    mbar_init(d_full, kTcG * kTcIss);
     mbar_init(d_empty, kTcGenWarps);
-    mbar_init(smem_u32(&sm.sink), 1);
+    mbar_init(sinkb, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == kTcGenWarps) tmem_alloc(smem_u32(&sm.tmem_base), kTcTmemCols);
@@ -134,9 +247,8 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
   __syncthreads();
   tc_fence_after();
   const unsigned tmem = sm.tmem_base;
-  // TMEM columns: D of group g at g * N; A buffer (g, buf) at kTcG * N + (a_bufs g + buf) * kTcACols
+  // TMEM columns: D of group g at g * N; A slot (g, s) at kTcG * N + (kTcABufs g + s) * kTcACols
   const unsigned a_col0 = (unsigned)(kTcG * N);
-  const unsigned nab = (unsigned)tp.a_bufs, nab_sh = (unsigned)tp.a_shift;   // A ring depth (power of two)
   // The accumulators start from zero and the epilogue leaves them zero again, so every MMA accumulates
   // and no MMA has to be the first of its tile.
   if (warp < kTcGenWarps) {
@@ -149,124 +261,196 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
   tc_fence_after();
 
   if (warp == kTcGenWarps) {
+    reg_dec<kTcRegsSvc>();
     // ===================================== TMA PRODUCER =======================================
     // A stage holds the windows of `qs` consecutive transmits of one receiver (one barrier round
     // per qs items).  Lane q works out the window of item (q, m), the union over the voxel groups,
-    // and issues its own bulk copy; lane 0 waits for the stage and posts the byte count.
+    // and issues its own bulk copy; lane 0 waits for the stage and posts the byte count.  Lane q also
+    // tells the MMA issuers what to do with item (q, m): one word per voxel group in the stage's info
+    // block (passes | offset of the group's window inside the staged one), published by the stage's
+    // full barrier.  Bit 31 of a stage's first info word marks the last stage of a tile.
     unsigned s = 0, ph = 0;                                  // stage and its phase parity
     const bool has_q = lane < P.Q;
+    TC_PROF_DECL
     for (int work = blockIdx.x; work < n_work; work += gridDim.x) {
       const int tile_i = work % tp.n_tiles, chunk = work / tp.n_tiles;
       const TcTile td = tp.tiles[tile_i];
-      const unsigned char* base = convb + (long long)chunk * chunk_bytes;
-      const int tb4 = __ldg(&tp.tbase[(long long)tile_i * P.Q + ql]) >> 2;       // k-block of tbase_q
-      // window of item (q = lane, m) of a list entry: byte offset inside the chunk and length; fetched
-      // one entry ahead (the loads are a dependent chain through L2)
-      auto entry_window = [&](const long long e, unsigned& any, unsigned& bytes) {
+      const int tb_q = __ldg(&tp.tbase[(long long)tile_i * P.Q + ql]);
+      // item (q = lane, m) of a list entry: first K row of its box (the union of the groups' windows), the
+      // tensor coordinate of its (m, q) record, and the issuers' info words; fetched one entry ahead (the
+      // loads are a dependent chain through L2)
+      struct Ent { unsigned any, bytes, inf[kTcG]; int c0, c2; bool big; };
+      auto entry_window = [&](const long long e) {
+        Ent r;
         const uint2 hd = __ldg(&tp.list[e]);
-        any = hd.y;
-        int wlo, wn;
-        tc_union_window(tp.codes + e * kTcG * 16 + ql, wlo, wn);
-        bytes = has_q ? (unsigned)wn * slab : 0u;
-        return ((long long)hd.x * P.Q * tp.KBp + kTcPadBlocks + (long long)ql * tp.KBp + tb4 + wlo) * (long long)slab;
+        r.any = hd.y;
+        int lo = 0x7fffffff;
+        unsigned c[kTcG];
+        bool used = false;
+        r.big = false;
+#pragma unroll
+        for (int g = 0; g < kTcG; ++g) {
+          c[g] = __ldg(&tp.codes[(e * kTcG + g) * 16 + ql]);
+          if (code_passes(c[g])) { lo = min(lo, code_start(c[g])); used = true; r.big = r.big || (c[g] & kTcCodeBig); }
+        }
+        if (!used) lo = 0;
+        // info word: passes | K-row offset of the group's window inside the box (16-byte units) << 2 | big box << 30
+#pragma unroll
+        for (int g = 0; g < kTcG; ++g)
+          r.inf[g] = has_q ? ((unsigned)code_passes(c[g]) | ((code_passes(c[g]) ? (unsigned)(2 * (code_start(c[g]) - lo)) : 0u) << 2) |
+                              (r.big ? 0x40000000u : 0u)) : 0u;
+        r.bytes = (has_q && used) ? (r.big ? stage_bytes : small_bytes) : 0u;
+        r.c0 = 8 * (tb_q + lo);                               // 32-bit elements: 4 per K row, 2 K rows per sample
+        r.c2 = (chunk * P.M + (int)hd.x) * P.Q + ql;
+        return r;
       };
-      unsigned any_n = 0, bytes_n = 0;
-      long long src_n = 0;
-      if (td.list_cnt) src_n = entry_window(td.list_off, any_n, bytes_n);
-      for (int li = 0; li < td.list_cnt; ++li) {
-        const unsigned any = any_n, bytes_l = bytes_n;
-        const long long src_l = src_n;
-        if (li + 1 < td.list_cnt) src_n = entry_window((long long)td.list_off + li + 1, any_n, bytes_n);
-        if (!any) continue;
+      // index of the last list entry any group uses (its last stage ends the tile for the issuers)
+      int last_li = -1;
+      for (int li0 = 0; li0 < td.list_cnt; li0 += 32) {
+        const int li = li0 + lane;
+        const bool used = li < td.list_cnt && __ldg(&tp.list[td.list_off + li]).y != 0u;
+        const unsigned m = __ballot_sync(0xffffffffu, used);
+        if (m) last_li = li0 + 31 - __clz(m);
+      }
+      Ent nx;
+      nx.any = 0; nx.bytes = 0; nx.c0 = 0; nx.c2 = 0; nx.big = false;
+      if (td.list_cnt) nx = entry_window(td.list_off);
+      bool sent = false;
+      for (int li = 0; li < td.list_cnt || !sent; ++li) {
+        Ent cur;
+        if (li < td.list_cnt) {
+          cur = nx;
+          if (li + 1 < td.list_cnt) nx = entry_window((long long)td.list_off + li + 1);
+          if (!cur.any) continue;
+        } else {
+          // a tile without any receiver: one empty stage, so that the issuers see the end of the tile
+          cur.any = 0; cur.bytes = 0; cur.c0 = 0; cur.c2 = 0; cur.big = false;
+#pragma unroll
+          for (int g = 0; g < kTcG; ++g) cur.inf[g] = 0u;
+        }
+        sent = true;
         for (int q0 = 0; q0 < P.Q; q0 += (int)qs) {
           const bool mine = lane >= q0 && lane < q0 + (int)qs;
-          const unsigned total = __reduce_add_sync(0xffffffffu, mine ? bytes_l : 0u);
+          const unsigned total = __reduce_add_sync(0xffffffffu, mine ? cur.bytes : 0u);
+          const bool last_stage = li >= last_li && q0 + (int)qs >= P.Q;
+          TC_PROF_WAIT(1, if (lane == 0) mbar_wait_park(b_empty0 + 8 * s, ph ^ 1u); __syncwarp())
+          __syncwarp();
+          if (mine) {
+#pragma unroll
+            for (int g = 0; g < kTcG; ++g)
+              sm.info[(s * kTcMaxQs + (unsigned)(lane - q0)) * kTcG + g] = cur.inf[g] | ((last_stage && lane == q0) ? 0x80000000u : 0u);
+          }
+          __syncwarp();
           if (lane == 0) {
-            mbar_wait_park(b_empty0 + 8 * s, ph ^ 1u);
             if (total) mbar_arrive_expect_tx(b_full0 + 8 * s, total);
             else mbar_arrive(b_full0 + 8 * s);
           }
           __syncwarp();
-          if (mine && bytes_l)
-            tma_bulk_g2s(stage0 + (s * qs + (unsigned)(lane - q0)) * stage_bytes, base + src_l, bytes_l, b_full0 + 8 * s);
+          if (mine && cur.bytes)
+            tma_tensor3_g2s(stage0 + (s * qs + (unsigned)(lane - q0)) * stage_bytes, cur.big ? &tmap_big : &tmap_small, cur.c0, 0, cur.c2, b_full0 + 8 * s);
           if (++s == (unsigned)tp.n_stages) { s = 0; ph ^= 1u; }
           __syncwarp();
         }
       }
     }
+    TC_PROF_END
+  } else if (warp > kTcGenWarps + kTcIss * kTcG) {
+    reg_dec<kTcRegsSvc>();                                   // idle warp (roles come in whole warpgroups: setmaxnreg)
   } else if (warp > kTcGenWarps) {
+    reg_dec<kTcRegsSvc>();
     // ===================================== MMA ISSUERS ========================================
     // One warp per voxel group.  The issue loop is a serial chain (wait -> MMA -> commit) whose
     // latency bounds the MMA rate of a group, so it is kept as short as it can be: lane q prepares
     // item (q, m) (passes, offset of the group's window inside the staged one), every lane runs the
     // same scalar loop (no divergence, one shuffle per item), only the tcgen05 instructions sit
-    // under an elected lane, and the stage barriers are visited once per qs items.
-    const int g = warp - kTcGenWarps - 1;
-    const unsigned idesc = tc_idesc(N);
-    const unsigned d_tmem = tmem + (unsigned)(g * N);
-    const unsigned a_tmem0 = tmem + a_col0 + (nab * (unsigned)g) * kTcACols;
-    const unsigned af0 = a_full0 + 8u * (nab * (unsigned)g), ae0 = a_empty0 + 8u * (nab * (unsigned)g);
-    // descriptor of a B tile at shared address 0: LBO = one slab (the two K chunks), SBO = 128 B
-    const unsigned long long desc0 = tc_smem_desc(0u, slab, 128);
-    unsigned s = 0, ph = 0, a_it = 0, n_done = 0;
-    for (int work = blockIdx.x; work < n_work; work += gridDim.x, ++n_done) {
-      const int tile_i = work % tp.n_tiles;
-      const TcTile td = tp.tiles[tile_i];
-      mbar_wait_park(d_empty, (n_done & 1u) ^ 1u);             // epilogue of the previous tile has drained D
-      tc_fence_after();
-      // item (q = lane, m) of a list entry: passes | 16-byte units from the start of the staged window to
-      // this group's window << 2; fetched one entry ahead (the loads are a dependent chain through L2)
-      auto entry_info = [&](const long long e, unsigned& any) {
-        any = __ldg(&tp.list[e]).y;
-        int wlo, wn;
-        tc_union_window(tp.codes + e * kTcG * 16 + ql, wlo, wn);
-        const unsigned c = __ldg(&tp.codes[(e * kTcG + g) * 16 + ql]);
-        return (unsigned)code_passes(c) | ((code_passes(c) ? (unsigned)((code_start2(c) >> 1) - wlo) * (slab >> 4) : 0u) << 2);
-      };
-      unsigned any_n = 0, info_n = 0;
-      if (td.list_cnt) info_n = entry_info(td.list_off, any_n);
-      for (int li = 0; li < td.list_cnt; ++li) {
-        const unsigned any = any_n, info_l = info_n;
-        if (li + 1 < td.list_cnt) info_n = entry_info((long long)td.list_off + li + 1, any_n);
-        if (!any) continue;
-        for (int q0 = 0; q0 < P.Q; q0 += (int)qs) {
-          mbar_wait_park(b_full0 + 8 * s, ph);                 // also keeps an idle group in step with the ring
-          const int q1 = min(q0 + (int)qs, P.Q);
-          for (int q = q0; q < q1; ++q) {
-            const unsigned info = __shfl_sync(0xffffffffu, info_l, q);
-            const int np = (int)(info & 3u);
-            unsigned long long desc = desc0 + (unsigned long long)(((stage0 + (s * qs + (unsigned)(q - q0)) * stage_bytes) >> 4) + (info >> 2));
-            for (int p = 0; p < np; ++p, ++a_it, desc += (unsigned long long)((kTcPassBlocks * slab) >> 4)) {
-              const unsigned buf = a_it & (nab - 1u);
-              mbar_wait_park(af0 + 8u * buf, (a_it >> nab_sh) & 1u);
+    // under an elected lane, and the stage barriers are visited once per qs items.  Item q takes
+    // its A tile from slot q mod 4, further passes from the overflow slot (das_tc.cuh).
+    const int g = (warp - kTcGenWarps - 1) / kTcIss;
+    const unsigned turn = (unsigned)((warp - kTcGenWarps - 1) % kTcIss);   // this warp issues the items with n_main mod kTcIss == turn
+    if (lane == 0) {
+      const unsigned idesc = tc_idesc(N);
+      const unsigned d_tmem = tmem + (unsigned)(g * N);
+      const unsigned a_tmem0 = tmem + a_col0 + (unsigned)(kTcABufs * g) * kTcACols;
+      const unsigned af0 = a_full0 + 8u * (unsigned)(kTcABufs * g), ae0 = a_empty0 + 8u * (unsigned)(kTcABufs * g);
+      // descriptor of a B tile at shared address 0: LBO = 8 K rows (the next core matrix along K), SBO = one
+      // column group of the box (its K rows: small or big box); only the 14-bit address field (bits 0-13 of the low
+      // word, 16-byte units = K rows) changes from MMA to MMA
+      const unsigned long long desc_s = tc_smem_desc(0u, 8 * 16, 2 * kTcBoxSmall * 16), desc_b = tc_smem_desc(0u, 8 * 16, 2 * kTcBoxBig * 16);
+      const unsigned desc_lo0 = (unsigned)desc_s, desc_hi_s = (unsigned)(desc_s >> 32), desc_hi_b = (unsigned)(desc_b >> 32);
+      const unsigned stage_u16 = stage_bytes >> 4, pass_u16 = 2 * kTcPass;   // K rows of one MMA pass
+      const unsigned info0 = smem_u32(&sm.info[0]) + 4u * (unsigned)g;
+      // n_main / n_ovf: MMAs issued so far from item tiles / overflow tiles.  Item tiles use their 4 slots
+      // round robin, so slot and barrier phase follow from the counter: slot = n mod 4, parity = (n / 4) mod 2.
+      unsigned s = 0, ph = 0, n_done = 0, n_main = 0, n_ovf = 0;
+      TC_PROF_DECL
+      for (int work = blockIdx.x; work < n_work; work += gridDim.x, ++n_done) {
+        TC_PROF_WAIT(1, mbar_wait_park(d_empty, (n_done & 1u) ^ 1u))           // epilogue of the previous tile has drained D
+        tc_fence_after();
+        bool last = false;
+        while (!last) {
+          TC_PROF_WAIT(2, mbar_wait_park(b_full0 + 8 * s, ph))
+          unsigned slot_u16 = (stage0 + s * qs * stage_bytes) >> 4;       // window slot of the item, 16-byte units
+          unsigned ia = info0 + s * (kTcMaxQs * kTcG * 4u);
+          unsigned info = lds_volatile(ia);
+          last = (info >> 31) != 0u;
+          info &= 0x7fffffffu;
+          for (unsigned i = 0; i < qs; ++i, slot_u16 += stage_u16) {
+            ia += kTcG * 4u;
+            const unsigned info_next = (i + 1 < qs) ? lds_volatile(ia) : 0u;   // one item ahead (slots beyond Q hold 0)
+            const unsigned np = info & 3u;
+            if (np && n_main % kTcIss != turn) {
+              n_ovf += np - 1u;
+              ++n_main;
+            } else if (np) {
+              const unsigned sl = n_main & (kTcSlots - 1);
+              unsigned dlo = desc_lo0 + slot_u16 + ((info >> 2) & 0xfffu);
+              const unsigned desc_hi = (info & 0x40000000u) ? desc_hi_b : desc_hi_s;
+              TC_PROF_WAIT(3, mbar_wait_park(af0 + 8u * sl, (n_main >> 2) & 1u))
               tc_fence_after();
-              if (tc_elect()) {
-                tc_mma_ts(d_tmem, a_tmem0 + buf * kTcACols, desc, idesc, 1u);
-                tc_commit(ae0 + 8u * buf);                     // A buffer free once this MMA has read it
+              TC_PROF_WAIT(5, tc_mma_ts(d_tmem, a_tmem0 + sl * kTcACols, ((unsigned long long)desc_hi << 32) | dlo, idesc, 1u))
+              TC_PROF_WAIT(6, tc_commit(ae0 + 8u * sl))                        // completes when this MMA has read its A slot
+              for (unsigned p = 1; p < np; ++p) {
+                dlo += pass_u16;
+                TC_PROF_WAIT(4, mbar_wait_park(af0 + 8u * kTcOvf, n_ovf & 1u))
+                ++n_ovf;
+                tc_fence_after();
+                tc_mma_ts(d_tmem, a_tmem0 + kTcOvf * kTcACols, ((unsigned long long)desc_hi << 32) | dlo, idesc, 1u);
+                tc_commit(ae0 + 8u * kTcOvf);
               }
+              ++n_main;
             }
+            info = info_next;
           }
-          if (tc_elect()) tc_commit(b_empty0 + 8 * s);         // this group is done with the stage
+          tc_commit(b_empty0 + 8 * s);                         // this group is done with the stage
           if (++s == (unsigned)tp.n_stages) { s = 0; ph ^= 1u; }
         }
+        tc_commit(d_full);                                     // this group's MMAs of the tile are complete
       }
-      if (tc_elect()) tc_commit(d_full);                       // this group's MMAs of the tile are complete
+      TC_PROF_END
     }
   } else {
     // ===================================== GENERATORS =========================================
+    reg_inc<kTcRegsGen>();
     const int g = warp >> 2;                                  // voxel group = depth inside the tile
     const int row = (warp & 3) * 32 + lane;                   // MMA row = TMEM lane (quarter warp % 4)
     const unsigned lane_base = ((unsigned)((warp & 3) * 32)) << 16;
     const unsigned d_addr = tmem + lane_base + (unsigned)(g * N);
-    const unsigned a_addr0 = tmem + lane_base + a_col0 + (nab * (unsigned)g) * kTcACols;
-    TcGenRing rg;
-    rg.a_it = 0;
-    rg.pend = smem_u32(&sm.sink);
-    rg.nab = nab; rg.nab_sh = nab_sh;
-    rg.ae0 = a_empty0 + 8u * (nab * (unsigned)g); rg.af0 = a_full0 + 8u * (nab * (unsigned)g);
-    rg.a_addr0 = a_addr0;
-    rg.lane0 = lane == 0;
+    TcGenState st;
+    asm volatile("mov.u32 %0, %1;" : "=r"(st.a_addr0) : "r"(tmem + lane_base + a_col0 + (unsigned)(kTcABufs * g) * kTcACols));
+    asm volatile("mov.u32 %0, %1;" : "=r"(st.ae0) : "r"(a_empty0 + 8u * (unsigned)(kTcABufs * g)));
+    asm volatile("mov.u32 %0, %1;" : "=r"(st.af0) : "r"(a_full0 + 8u * (unsigned)(kTcABufs * g)));
+    st.sink = sinkb;
+    st.pend = sinkb;
+    st.it = 0u;
+    st.par = 0u;
+    st.free_next = false;
+    st.ovf_pend = false;
+    st.lane0 = lane == 0;
     unsigned n_done = 0;
+    TC_PROF_DECL
+#ifdef DAS_TC_PROF
+    st.pf1 = st.pf2 = st.pf3 = 0;
+#endif
 
     for (int work = blockIdx.x; work < n_work; work += gridDim.x, ++n_done) {
       const int tile_i = work % tp.n_tiles, chunk = work / tp.n_tiles;
@@ -313,21 +497,37 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
         // per-(m, n): aperture, excess path, receive phase (as in das_tiled.cuh)
         bool act;
         const float ex = tc_excess(tp, P, vx, el, act);
+        if (!__any_sync(0xffffffffu, act)) {
+          // no voxel of this WARP sees the receiver: 32 zero rows per item, no arithmetic
+          if (q16) tc_gen_receiver<false, true, true>(Tf, pc, ps, 0.f, 0.f, 0.f, cw0, cw1, tb_l, P.Q, P.K, st);
+          else tc_gen_receiver<false, true, false>(Tf, pc, ps, 0.f, 0.f, 0.f, cw0, cw1, tb_l, P.Q, P.K, st);
+          continue;
+        }
         float cyc = tp.ratio_f * ex;
         cyc -= rintf(cyc);
         const float ang = 6.283185307179586f * cyc;
         const float pr = act ? cos_approx(ang) : 0.f, pi = act ? sin_approx(ang) : 0.f;
-        if (td.edge) tc_gen_receiver<true>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, rg);
-        else tc_gen_receiver<false>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, rg);
+        if (q16) {
+          if (td.edge) tc_gen_receiver<true, false, true>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, st);
+          else tc_gen_receiver<false, false, true>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, st);
+        } else {
+          if (td.edge) tc_gen_receiver<true, false, false>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, st);
+          else tc_gen_receiver<false, false, false>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, st);
+        }
       }
       tmem_wait_st();
       tc_fence_before();
-      if (rg.lane0) mbar_arrive(rg.pend);
-      rg.pend = smem_u32(&sm.sink);
+      mbar_arrive_if(st.pend, st.lane0);
+      mbar_arrive_if(st.af0 + 8u * kTcOvf, st.lane0 && st.ovf_pend);
+      st.pend = sinkb;
+      st.ovf_pend = false;
 
       // ---- epilogue: D (FP32, TMEM) -> out[frame][voxel] -------------------------------------
-      mbar_wait_park(d_full, n_done & 1u);
+      TC_PROF_WAIT(3, mbar_wait_park(d_full, n_done & 1u))
       tc_fence_after();
+#ifdef DAS_TC_PROF
+      const long long ep0_ = clock64();
+#endif
       const long long vox = ((long long)vx.ix * P.ny + vx.iy) * P.nz + vx.iz;
       float2* dst = out + (long long)chunk * tp.Bc * n_vox + vox;
       for (int c0 = 0; c0 < N; c0 += 16) {
@@ -346,7 +546,14 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(d_empty);
+#ifdef DAS_TC_PROF
+      pf_[4] += (unsigned long long)(clock64() - ep0_);
+#endif
     }
+#ifdef DAS_TC_PROF
+    pf_[1] = st.pf1; pf_[2] = st.pf2; pf_[5] = st.pf3;
+#endif
+    TC_PROF_END
   }
 
   tc_fence_before();
@@ -359,9 +566,13 @@ tc_kernel(const TcDev tp, const Params P, const unsigned char* __restrict__ conv
 // One CTA per tile, thread = (voxel group, MMA row).  For every listed receiver m and transmit q
 // it takes the minimum and maximum of floor(t_qmn) over the ACTIVE voxels of each group, with the
 // same FP32 arithmetic as the generator warps (tc_voxel / tc_T / tc_excess) widened by kTcDelta,
-// and writes the window code the three warp roles of tc_kernel read (TcDev::codes).
-//   stats[0] = largest staged window (k-blocks), stats[1] = error bits
-//   (1: window needs more than 3 passes, 2: window leaves the zero pads, 4: negative start)
+// and writes the window code the warp roles of tc_kernel read (TcDev::codes): a group needs the
+// samples [smin, smax + 1], i.e. ceil((smax + 2 - smin) / 8) MMA passes from sample smin on.  The
+// windows of the groups of one (entry, q) must lie in one box (kTcBoxSmall samples if every group needs one
+// pass and the item needs no more than that, else kTcBoxBig) starting at the smallest smin: a window that
+// would stick out of the box is moved down (it then starts before its smin, which costs nothing).
+//   stats[0] = largest number of samples one (entry, q) needs, stats[1] = error bits
+//   (1: a group needs more than 2 passes, 2: the groups of an item do not fit one box, 4: negative start)
 __global__ void __launch_bounds__(kTcG * kTcRows)
 tc_window_kernel(const TcDev tp, const Params P, uint2* __restrict__ list, unsigned short* __restrict__ codes,
                  int* __restrict__ tile_work, int* __restrict__ tile_edge, int* __restrict__ stats) {
@@ -370,15 +581,14 @@ tc_window_kernel(const TcDev tp, const Params P, uint2* __restrict__ list, unsig
   const int g = tid / kTcRows, row = tid % kTcRows;
   const TcTile td = tp.tiles[tile_i];
   const TcVoxel vx = tc_voxel(tp, P, td, row, g);
-  const int Kb = (P.K + kTcBlk - 1) / kTcBlk;
   float Tf[16];
 #pragma unroll
   for (int q = 0; q < 16; ++q) {
     const int qq = min(q, P.Q - 1);
     Tf[q] = (float)(tc_T(P, vx, qq) - (double)__ldg(&tp.tbase[(long long)tile_i * P.Q + qq]));
   }
-  const int tb4 = tid < 16 ? (__ldg(&tp.tbase[(long long)tile_i * P.Q + min(tid, P.Q - 1)]) >> 2) : 0;
-  int work = 0, edge = 0, stage = 0, err = 0;
+  const int tb = tid < 16 ? __ldg(&tp.tbase[(long long)tile_i * P.Q + min(tid, P.Q - 1)]) : 0;
+  int work = 0, edge = 0, span = 0, err = 0;
 
   for (int li = 0; li < td.list_cnt; ++li) {
     const long long e = td.list_off + li;
@@ -400,29 +610,35 @@ tc_window_kernel(const TcDev tp, const Params P, uint2* __restrict__ list, unsig
     __syncthreads();
     if (tid < 16) {
       const int q = tid;
-      int wlo = INT_MAX, whi = INT_MIN;
       unsigned flags = 0;
+      int u0 = INT_MAX, uend = INT_MIN;                          // samples the item needs: [u0, uend)
+      if (q < P.Q)
+        for (int gg = 0; gg < kTcG; ++gg)
+          if (kmn[gg][q] != INT_MAX) { u0 = min(u0, kmn[gg][q]); uend = max(uend, kmx[gg][q] + 2); }
+      bool big = false;
+      if (u0 != INT_MAX) {
+        big = uend - u0 > kTcBoxSmall;
+        for (int gg = 0; gg < kTcG; ++gg)
+          if (kmn[gg][q] != INT_MAX && kmx[gg][q] + 2 - kmn[gg][q] > kTcPass) big = true;   // a two-pass window needs 16 samples
+        if (u0 < 0 || u0 > 0x1fff - kTcBoxBig) err |= 4;
+        if (uend - u0 > kTcBoxBig) err |= 2;
+        span = max(span, uend - u0);
+        if (tb + u0 <= 0 || tb + u0 + kTcBoxBig >= P.K - 1) edge = 1;
+      }
+      const int box = big ? kTcBoxBig : kTcBoxSmall;
       for (int gg = 0; gg < kTcG; ++gg) {
         unsigned code = 0;
         if (q < P.Q && kmn[gg][q] != INT_MAX) {
           const int smin = kmn[gg][q], smax = kmx[gg][q];
-          if (smin < 0) err |= 4;
-          const int b0 = max(smin, 0) >> 2;
-          const int nb = ((smax + 1) >> 2) - b0 + 1;
-          const int np = (nb + kTcPassBlocks - 1) / kTcPassBlocks;
-          if (np > 3 || b0 * 2 > 0x3fff) err |= 1;
-          code = (unsigned)min(np, 3) | ((unsigned)(b0 * 2) << 2);
-          wlo = min(wlo, tb4 + b0);
-          whi = max(whi, tb4 + b0 + kTcPassBlocks * np);
+          const int np = (smax + 2 - smin + kTcPass - 1) / kTcPass;
+          if (np > 2) err |= 1;
+          const int npc = min(np, 2);
+          const int start = max(min(smin, u0 + box - kTcPass * npc), 0);
+          code = (unsigned)npc | ((unsigned)min(start, 0x1fff) << 2) | (big ? (unsigned)kTcCodeBig : 0u);
           flags |= 1u << gg;
-          work += np;
+          work += npc;
         }
         codes[(e * kTcG + gg) * 16 + q] = (unsigned short)code;
-      }
-      if (whi > wlo) {
-        stage = max(stage, whi - wlo);
-        if (wlo < -kTcPadBlocks || whi > Kb + kTcPadBlocks) err |= 2;
-        if (kTcBlk * wlo <= 0 || kTcBlk * whi >= P.K - 1) edge = 1;
       }
       flags = __reduce_or_sync(0x0000ffffu, flags);
       if (tid == 0) list[e].y = flags;
@@ -432,12 +648,12 @@ tc_window_kernel(const TcDev tp, const Params P, uint2* __restrict__ list, unsig
   if (tid < 16) {
     work = __reduce_add_sync(0x0000ffffu, work);
     edge = __reduce_or_sync(0x0000ffffu, edge);
-    stage = __reduce_max_sync(0x0000ffffu, stage);
+    span = __reduce_max_sync(0x0000ffffu, span);
     err = __reduce_or_sync(0x0000ffffu, err);
     if (tid == 0) {
       tile_work[tile_i] = work;
       tile_edge[tile_i] = edge;
-      atomicMax(&stats[0], stage);
+      atomicMax(&stats[0], span);
       if (err) atomicOr(&stats[1], err);
     }
   }
@@ -451,14 +667,12 @@ cudaError_t launch_tc_windows(const TcDev& tp, const Params& P, uint2* list, uns
   return cudaGetLastError();
 }
 
-cudaError_t launch_tc_kernel(const TcDev& tp, const Params& P, const void* d_conv, void* d_out, int grid, size_t smem, cudaStream_t s) {
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
-  tc_kernel<<<grid, kTcThreads, smem, s>>>(tp, P, static_cast<const unsigned char*>(d_conv), static_cast<float2*>(d_out));
+cudaError_t launch_tc_kernel(const TcDev& tp, const Params& P, const void* tmaps, void* d_out, int grid, size_t smem, cudaStream_t s) {
+  // per launch: the attribute belongs to the (device, context) the plan lives on, and it is cheap
+  cudaError_t e = cudaFuncSetAttribute(tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024 + 2048);
+  if (e != cudaSuccess) return e;
+  const CUtensorMap* maps = static_cast<const CUtensorMap*>(tmaps);                  // [0] small box, [1] big box
+  tc_kernel<<<grid, kTcThreads, smem, s>>>(tp, P, maps[0], maps[1], static_cast<float2*>(d_out));
   return cudaGetLastError();
 }
 

@@ -19,7 +19,7 @@
 // complex product).  A is GENERATED per (q, m, voxel) on the CUDA cores (FP32 arithmetic, FP64
 // for the part common to all receivers exactly as in das_tiled.cuh), rounded to FP16 and
 // written straight into tensor memory; Y is the converted channel data (das_convert, batch
-// layout) staged in shared memory by TMA bulk copies; D accumulates in FP32 in tensor memory
+// layout) staged in shared memory by TMA tensor copies; D accumulates in FP32 in tensor memory
 // over all transmits and receivers of a voxel tile.  The weights are amortised over the Bc
 // frames of a chunk: the per-frame cost on the CUDA cores drops by Bc.
 //
@@ -28,10 +28,19 @@
 //                = TMEM lane.  Per receiver: aperture test, excess path, receive phase.  Per
 //                (q, m): fractional index, weights, the 8 packed FP16 pairs of an A row ->
 //                tcgen05.st.  After the last receiver: tcgen05.ld of D -> global, D zeroed again.
+//                The A tiles of a group live in a ring of 4 ITEM SLOTS in tensor memory plus one
+//                OVERFLOW slot: item q of a receiver always uses slot q mod 4 (first MMA pass of its
+//                window), the 2nd / 3rd pass of the 30 % of items that need one goes through the
+//                overflow slot.  Slot, barrier address and (for 16 transmits) barrier phase of every
+//                item are therefore compile-time constants in the unrolled transmit loop: one
+//                mbarrier round per item with no ring arithmetic.
 //   warp 12      TMA producer: one bulk copy per (q, m) of the k-blocks the tile needs.
-//   warps 13..15 MMA issuers, one per voxel group: tcgen05.mma.kind::f16, A from TMEM, B from
-//                shared memory (K-major, no swizzle: a k-block of N columns x 16 B is one slab),
-//                D of the group in TMEM.  The issue loop is a serial latency chain (wait, MMA,
+//   warps 13..18 MMA issuers, two per voxel group: tcgen05.mma.kind::f16, A from TMEM, B from
+//                shared memory, D of the group in TMEM.  B is MN-MAJOR without swizzle: a K row is one
+//                (sample, y | -j y) vector over the N = 2 Bc frame columns, stored as N / 8 column
+//                groups of 16 bytes; per column group the K rows are contiguous, so an MMA window
+//                (8 samples = 16 K rows = two 8-row core matrices) may start at ANY sample of the
+//                staged box: the descriptor's start address moves in steps of one row pair.  The issue loop is a serial latency chain (wait, MMA,
 //                commit): every lane runs it, only the tcgen05 instructions sit under elect.sync.
 //   (The issue arbiter favours high warp ids: the short, latency-critical service warps sit above
 //   the generators; the other order measured 5 % slower.)
@@ -44,21 +53,32 @@ namespace das {
 constexpr int kTcGX = 16, kTcGY = 8;        // a voxel group: 16 x 8 lateral voxels at one depth
 constexpr int kTcRows = kTcGX * kTcGY;      // = 128 = MMA M
 constexpr int kTcG = 3;                     // voxel groups (consecutive depths) per tile
-constexpr int kTcBlk = 4;                   // samples per k-block (8 FP16 = 16 B per column)
-constexpr int kTcPassBlocks = 2;            // k-blocks per pass = one MMA of K = 16
-constexpr int kTcMaxABufs = 8;              // A ring per voxel group (TMEM), one MMA each; depth a power of two
+constexpr int kTcBlk = 4;                   // samples per core matrix of the B operand (8 K rows: y and -j y of 4 samples)
+constexpr int kTcPassBlocks = 2;            // core matrices per pass = one MMA of K = 16 = 8 samples
+constexpr int kTcPass = kTcBlk * kTcPassBlocks;   // samples per MMA pass
+// One staged box (a TMA tensor copy) holds the union of the windows of a tile's voxel groups for one (q, m).
+// Two box sizes: the small one takes the common case (every group one MMA pass, 87 % of the items at the
+// headline), the big one the rest; the stage slot has the big one's size.
+constexpr int kTcBoxSmall = 12, kTcBoxBig = 20;   // samples
+constexpr int kTcCodeBig = 0x8000;                // window code: the item uses the big box
+constexpr int kTcSlots = 4;                 // item slots of a group's A ring (TMEM): item q uses slot q mod 4
+constexpr int kTcOvf = kTcSlots;            // the overflow slot: 2nd / 3rd MMA pass of an item
+constexpr int kTcABufs = kTcSlots + 1;      // A tiles per voxel group in tensor memory
 constexpr int kTcMaxStages = 16;            // upper bound of the shared-memory ring of staged sample windows
 constexpr int kTcMinStages = 2;
-constexpr int kTcPadBlocks = 16;            // zero k-blocks before and after every (m, q) row
-constexpr int kTcMaxStageBlocks = 16;       // largest window (k-blocks) one stage can hold
+constexpr int kTcMaxQs = 16;                // upper bound of the window slots (transmits) per stage
 constexpr int kTcGenWarps = 4 * kTcG;
-constexpr int kTcSvcWarps = 1 + kTcG;        // TMA producer + one MMA issuer per voxel group
+constexpr int kTcIss = 2;                    // MMA issuer warps per voxel group: the issue chain of one warp
+                                             // (~45 instructions per MMA at single-warp latency) caps a group
+                                             // at one MMA per ~400 cycles; the issuers take the items in turn
+constexpr int kTcSvcWarps = 8;               // TMA producer + kTcIss issuers per voxel group (+ idle: whole warpgroups)
 constexpr int kTcThreads = (kTcSvcWarps + kTcGenWarps) * 32;
+constexpr int kTcRegsGen = 128, kTcRegsSvc = 40;   // setmaxnreg: 12 x 32 x 128 + 8 x 32 x 40 <= 65536
+static_assert(1 + kTcIss * kTcG <= kTcSvcWarps && kTcSvcWarps % 4 == 0 && kTcGenWarps % 4 == 0, "warpgroup roles");
 constexpr int kTcTmemCols = 512;
 constexpr int kTcACols = 8;                 // TMEM columns of one A buffer (K = 16 FP16 per row)
 constexpr float kTcMargin = 0.02f;          // samples: slack of the plan's transmit-delay bounds (tbase)
 
-__host__ __device__ inline int tc_kblocks(int K) { return 2 * kTcPadBlocks + (K + kTcBlk - 1) / kTcBlk; }
 
 struct TcTile {
   int ix0, iy0, iz0;
@@ -69,43 +89,28 @@ struct TcTile {
 struct TcDev {
   int n_tiles, n_chunks;       // work items = n_tiles * n_chunks
   int Bc;                      // frames per chunk; MMA N = 2 Bc
-  int KBp;                     // k-blocks per (m, q) row of the converted data, pads included
-  int stage_blocks;            // capacity of one window slot in k-blocks
+  int groups;                  // depths per tile that carry voxels: kTcG, or 1 when the depths of the grid lie so
+                               // far apart in delay that the windows of kTcG of them do not fit one staged box
   int qs;                      // window slots (consecutive transmits of one receiver) per stage: one barrier round per qs items
   int n_stages;                // depth of the stage ring (kTcMinStages..kTcMaxStages)
-  int a_bufs, a_shift;         // depth of the A ring per voxel group (2^a_shift <= kTcMaxABufs, what TMEM holds)
   const TcTile* tiles;         // [n_tiles], sorted by decreasing work
-  const int* tbase;            // [n_tiles][Q]: sample offset of the reduced delays, multiple of 4
+  const int* tbase;            // [n_tiles][Q]: sample offset of the reduced delays
   const uint2* list;           // receiver lists of the tiles: x = m, y = bit g set if group g has a window
   const unsigned short* codes; // [entry][G][16]: window of item (q, m) for group g, written by the plan's
                                //   window kernel from the delays of the group's ACTIVE voxels:
                                //   bits 0-1 = n_pass (MMAs of K = 16 = 8 samples; 0 = no active voxel),
-                               //   bits 2-15 = first sample of the window in units of 2 samples, relative
-                               //   to tbase_q
+                               //   bits 2-14 = first sample of the window relative to tbase_q, bit 15 = the
+                               //   item (entry, q) uses the big box.  The windows of the groups of one
+                               //   (entry, q) lie inside one box that starts at the smallest of their first samples.
   double z_array, kappa, ratio, phase0;
   float four_f2, kappa_f, ratio_f;
+  unsigned long long* prof;    // cycle accounting per (CTA, warp), only in -DDAS_TC_PROF builds (else nullptr)
 };
 
 constexpr float kTcDelta = 1.0f / 128;      // samples: the window kernel widens every delay by this much, so that
                                             // rounding differences between it and the generator cannot matter
 __host__ __device__ inline int code_passes(unsigned c) { return (int)(c & 3u); }
-__host__ __device__ inline int code_start2(unsigned c) { return (int)(c >> 2); }   // units of 2 samples
-
-// Window of item (q, m) the producer stages: the union over the voxel groups, as (first k-block relative
-// to tbase_q / 4, number of k-blocks).  `codes_q` points at the code of group 0 for this q.
-__device__ __forceinline__ void tc_union_window(const unsigned short* codes_q, int& wlo, int& wn) {
-  int lo = 0x7fffffff, hi = -0x7fffffff;
-#pragma unroll
-  for (int g = 0; g < kTcG; ++g) {
-    const unsigned c = __ldg(&codes_q[g * 16]);
-    if (code_passes(c)) {
-      lo = min(lo, code_start2(c) >> 1);
-      hi = max(hi, (code_start2(c) >> 1) + kTcPassBlocks * code_passes(c));
-    }
-  }
-  wlo = hi > lo ? lo : 0;
-  wn = hi > lo ? hi - lo : 0;
-}
+__host__ __device__ inline int code_start(unsigned c) { return (int)((c >> 2) & 0x1fffu); }     // samples, relative to tbase_q
 
 // ---- geometry shared by the generator warps and the plan's window kernel ---------------------
 struct TcVoxel {
@@ -118,7 +123,7 @@ struct TcVoxel {
 __device__ __forceinline__ TcVoxel tc_voxel(const TcDev& tp, const Params& P, const TcTile& td, int row, int g) {
   TcVoxel v;
   v.ix = td.ix0 + row % kTcGX; v.iy = td.iy0 + row / kTcGX; v.iz = td.iz0 + g;
-  v.in_grid = v.ix < P.nx && v.iy < P.ny && v.iz < P.nz;
+  v.in_grid = v.ix < P.nx && v.iy < P.ny && v.iz < P.nz && g < tp.groups;
   v.izc = min(v.iz, P.nz - 1);
   v.x = P.xs[min(v.ix, P.nx - 1)]; v.y = P.ys[min(v.iy, P.ny - 1)]; v.z = P.zs[v.izc];
   v.a_d = (double)v.z - tp.z_array;
@@ -183,6 +188,18 @@ __device__ __forceinline__ void tc_mma_ts(unsigned d_tmem, unsigned a_tmem, unsi
       "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
       ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
 }
+// The same MMA followed by a tcgen05.commit to `bar`, both under ONE elected lane and in one block (the
+// elect / vote / uniform-register traffic of two separate elected statements doubled the issue chain).
+__device__ __forceinline__ void tc_mma_commit(unsigned d_tmem, unsigned a_tmem, unsigned desc_lo, unsigned desc_hi, unsigned idesc, unsigned bar) {
+  asm volatile(
+      "{\n\t.reg .pred p, q;\n\t.reg .b64 dsc;\n\t"
+      "mov.b64 dsc, {%2, %3};\n\t"
+      "setp.ne.b32 q, %4, 0;\n\t"
+      "elect.sync _|p, 0xffffffff;\n\t"
+      "@p tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], dsc, %4, q;\n\t"
+      "@p tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%5];\n\t}"
+      ::"r"(d_tmem), "r"(a_tmem), "r"(desc_lo), "r"(desc_hi), "r"(idesc), "r"(bar) : "memory");
+}
 __device__ __forceinline__ void tmem_st8(unsigned taddr, const unsigned (&v)[8]) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
                ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]) : "memory");
@@ -198,16 +215,23 @@ __device__ __forceinline__ void tmem_ld16(unsigned taddr, float (&v)[16]) {
                  "=f"(v[8]), "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15])
                : "r"(taddr) : "memory");
 }
-// shared-memory matrix descriptor, K-major, no swizzle: 8-row core matrices of 16-byte rows;
-// SBO = byte step between 8-column groups (N direction), LBO = byte step between the two
-// 16-byte K chunks of a K = 16 MMA (here: one slab = one k-block)
+// Shared-memory matrix descriptor of the B operand, MN-major, no swizzle ("interleave"): the canonical
+// layout is ((8 columns), n column groups) x ((8 K rows), k row groups) with 16-byte units, the 8 K rows of
+// a core matrix contiguous;  SBO = byte step between column groups, LBO = byte step between the two
+// 8-row groups of a K = 16 MMA.  Bit 46: descriptor version of sm_100.
 __device__ __forceinline__ unsigned long long tc_smem_desc(unsigned addr, unsigned lbo_bytes, unsigned sbo_bytes) {
   return (unsigned long long)((addr >> 4) & 0x3FFFu) | ((unsigned long long)((lbo_bytes >> 4) & 0x3FFFu) << 16) |
          ((unsigned long long)((sbo_bytes >> 4) & 0x3FFFu) << 32) | (1ull << 46);
 }
-// instruction descriptor: D = F32, A = B = F16, both K-major, dense, M = 128, N = n
+// instruction descriptor: D = F32, A = B = F16, A K-major (tensor memory), B MN-major (bit 16), dense, M = 128, N = n
 __host__ __device__ inline unsigned tc_idesc(int n) {
-  return (1u << 4) | ((unsigned)(n >> 3) << 17) | ((unsigned)(kTcRows >> 4) << 24);
+  return (1u << 4) | (1u << 16) | ((unsigned)(n >> 3) << 17) | ((unsigned)(kTcRows >> 4) << 24);
+}
+// TMA tensor copy (3-D tile) global -> this CTA's shared memory, completion (bytes) counted on an mbarrier;
+// elements outside the tensor read as zero
+__device__ __forceinline__ void tma_tensor3_g2s(unsigned dst, const void* tmap, int c0, int c1, int c2, unsigned bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+               ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
 }
 __device__ __forceinline__ unsigned pack_half2(float lo, float hi) {
   unsigned r;
@@ -217,14 +241,17 @@ __device__ __forceinline__ unsigned pack_half2(float lo, float hi) {
 
 struct alignas(128) TcSmemHeader {
   unsigned long long b_full[kTcMaxStages], b_empty[kTcMaxStages];
-  unsigned long long a_full[kTcG * kTcMaxABufs], a_empty[kTcG * kTcMaxABufs];
+  unsigned long long a_full[kTcG * kTcABufs], a_empty[kTcG * kTcABufs];
   unsigned long long d_full, d_empty;
   unsigned long long sink;           // arrivals nobody waits for (no A tile in flight)
+  unsigned info[kTcMaxStages * kTcMaxQs * kTcG];   // per stage and window slot: what each group's issuer does with the item
   unsigned tmem_base;
 };
 
-__host__ __device__ inline size_t tc_smem_bytes(int Bc, int stage_blocks, int qs, int n_stages) {
-  return sizeof(TcSmemHeader) + 128 + (size_t)n_stages * qs * stage_blocks * (2 * Bc) * 16;
+// bytes of one staged box: N / 8 column groups x 2 K rows per sample x 16 bytes
+__host__ __device__ inline unsigned tc_box_bytes(int Bc, int samples) { return (unsigned)(2 * Bc / 8) * (unsigned)(2 * samples) * 16u; }
+__host__ __device__ inline size_t tc_smem_bytes(int Bc, int qs, int n_stages) {
+  return sizeof(TcSmemHeader) + 1024 + (size_t)n_stages * qs * tc_box_bytes(Bc, kTcBoxBig);
 }
 
 struct TcPlan;

@@ -8,11 +8,13 @@
 #include <numeric>
 #include <vector>
 
+#include <cuda.h>
+
 #include "das_tc.cuh"
 
 namespace das {
 
-cudaError_t launch_tc_kernel(const TcDev& tp, const Params& P, const void* d_conv, void* d_out, int grid, size_t smem, cudaStream_t s);
+cudaError_t launch_tc_kernel(const TcDev& tp, const Params& P, const void* tmap, void* d_out, int grid, size_t smem, cudaStream_t s);
 
 struct TcPlan {
   TcDev dev{};
@@ -28,8 +30,9 @@ void tc_plan_destroy(TcPlan* tp) {
   delete tp;
 }
 
+// [chunk][m][q][N / 8 column groups][2 K rows][8 columns] FP16
 size_t tc_converted_bytes(const TcPlan* tp, const Params& P) {
-  return (size_t)tp->dev.n_chunks * P.M * P.Q * tp->dev.KBp * (size_t)(2 * tp->dev.Bc) * 16;
+  return (size_t)tp->dev.n_chunks * P.M * P.Q * (size_t)(2 * tp->dev.Bc / 8) * (2 * (size_t)P.K) * 16;
 }
 int tc_frames_per_chunk(const TcPlan* tp) { return tp->dev.Bc; }
 
@@ -46,13 +49,28 @@ cudaError_t up(TcPlan* tp, const std::vector<T>& h, const T** d_out) {
 }
 }  // namespace
 
+static TcPlan* tc_plan_create_groups(const Params& P, const das_plan_desc_t& d, int n_frames, int device, char* why,
+                                     size_t why_len, cudaError_t* cuda_err, int groups, bool* retry_narrow);
+
 TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, int device, char* why,
                        size_t why_len, cudaError_t* cuda_err) {
+  // kTcG consecutive depths per tile share the staged samples; if the depths of the grid are so far apart in
+  // delay that their windows do not fit one box, one depth per tile still works (the other groups stay empty)
+  bool retry = false;
+  TcPlan* tp = tc_plan_create_groups(P, d, n_frames, device, why, why_len, cuda_err, kTcG, &retry);
+  if (!tp && retry && *cuda_err == cudaSuccess) tp = tc_plan_create_groups(P, d, n_frames, device, why, why_len, cuda_err, 1, &retry);
+  return tp;
+}
+
+static TcPlan* tc_plan_create_groups(const Params& P, const das_plan_desc_t& d, int n_frames, int device, char* why,
+                                     size_t why_len, cudaError_t* cuda_err, int groups, bool* retry_narrow) {
   *cuda_err = cudaSuccess;
+  *retry_narrow = false;
   auto refuse = [&](const char* msg) -> TcPlan* { snprintf(why, why_len, "%s", msg); return nullptr; };
   // ---- applicability ------------------------------------------------------------------------
   if (!P.iq || !P.fp16) return refuse("the tensor-core path needs IQ data in fp16 storage");
   if (d.n_tx > 16) return refuse("more than 16 transmits");
+  if (d.n_samples < 2 * kTcBoxBig) return refuse("fewer samples per trace than two staged boxes");
   if (n_frames < 8 || n_frames % 8) return refuse("frame count is not a multiple of 8");
   int Bc = n_frames;
   if (n_frames > 64) { if (n_frames % 64) return refuse("frame count above 64 is not a multiple of 64"); Bc = 64; }
@@ -70,7 +88,7 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
   const bool apod = fnum > 0.0;
   const double kappa = fs / c;
   const int Q = d.n_tx, M = d.n_elem;
-  const int ntx = (d.nx + kTcGX - 1) / kTcGX, nty = (d.ny + kTcGY - 1) / kTcGY, ntz = (d.nz + kTcG - 1) / kTcG;
+  const int ntx = (d.nx + kTcGX - 1) / kTcGX, nty = (d.ny + kTcGY - 1) / kTcGY, ntz = (d.nz + groups - 1) / groups;
   const long long n_tiles_ll = (long long)ntx * nty * ntz;
   if (n_tiles_ll > (1 << 22)) return refuse("too many tiles");
   const int n_tiles = (int)n_tiles_ll;
@@ -87,10 +105,10 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
     for (int ty = 0; ty < nty; ++ty)
       for (int txi = 0; txi < ntx; ++txi, ++t) {
         TcTile& td = tiles[t];
-        td.ix0 = txi * kTcGX; td.iy0 = ty * kTcGY; td.iz0 = tz * kTcG;
+        td.ix0 = txi * kTcGX; td.iy0 = ty * kTcGY; td.iz0 = tz * groups;
         td.edge = 0;
         const int ix1 = std::min(td.ix0 + kTcGX, d.nx), iy1 = std::min(td.iy0 + kTcGY, d.ny);
-        const int iz1 = std::min(td.iz0 + kTcG, d.nz);
+        const int iz1 = std::min(td.iz0 + groups, d.nz);
         double xlo = 1e300, xhi = -1e300, ylo = 1e300, yhi = -1e300;
         for (int i = td.ix0; i < ix1; ++i) { xlo = std::min(xlo, (double)d.xs[i]); xhi = std::max(xhi, (double)d.xs[i]); }
         for (int i = td.iy0; i < iy1; ++i) { ylo = std::min(ylo, (double)d.ys[i]); yhi = std::max(yhi, (double)d.ys[i]); }
@@ -116,8 +134,8 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
         // receivers whose aperture cone can reach a voxel of the tile (bounding-box test; the window
         // kernel below classifies every voxel exactly and drops the receivers no group sees)
         td.list_off = (int)list.size();
-        const double a_max = (double)d.zs[iz1 - 1] - z_a, a_min = (double)d.zs[td.iz0] - z_a;
-        const double a_far = std::max(a_max, a_min);
+        double a_far = 0.0;                                   // deepest plane of the tile (the axis need not be monotonic)
+        for (int k = td.iz0; k < iz1; ++k) a_far = std::max(a_far, (double)d.zs[k] - z_a);
         for (int m = 0; m < M; ++m) {
           const double ex = d.elem_pos[3 * m], ey = d.elem_pos[3 * m + 1];
           const double nx_ = std::max(std::max(xlo - ex, ex - xhi), 0.0), ny_ = std::max(std::max(ylo - ey, ey - yhi), 0.0);
@@ -137,10 +155,11 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
   TcDev& dv = tp->dev;
   dv.n_tiles = n_tiles;
   dv.Bc = Bc;
+  dv.groups = groups;
   dv.n_chunks = n_frames / Bc;
-  dv.KBp = tc_kblocks(P.K);
   dv.z_array = z_a; dv.kappa = kappa; dv.ratio = fc / fs;
   dv.phase0 = fc * t_start - std::floor(fc * t_start);
+  dv.prof = nullptr;
   dv.four_f2 = (float)(4.0 * fnum * fnum);
   dv.kappa_f = (float)kappa; dv.ratio_f = (float)(fc / fs);
 
@@ -174,17 +193,14 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
   auto refuse_free = [&](const char* msg) -> TcPlan* { tc_plan_destroy(tp); return refuse(msg); };
   if (getenv("DAS_TC_VERBOSE")) {
     long long tw = 0; for (int w_ : work) tw += w_;
-    fprintf(stderr, "[das tc plan] tiles %d, list entries %zu, MMA passes %lld, largest window %d k-blocks\n", n_tiles, list.size(), tw, stats[0]);
+    fprintf(stderr, "[das tc plan] tiles %d, list entries %zu, MMA passes %lld, widest item %d samples, error bits %d\n", n_tiles, list.size(), tw, stats[0], stats[1]);
   }
-  if (stats[1] & 1) return refuse_free("a sample window of a voxel group needs more than 3 MMA passes (grid too coarse)");
-  if (stats[1] & 2) return refuse_free("a sample window leaves the zero-padded record");
-  if (stats[1] & 4) return refuse_free("internal: negative window start");
-  const int stage_blocks = std::max(stats[0], kTcPassBlocks);
-  if (stage_blocks > kTcMaxStageBlocks) {
-    snprintf(why, why_len, "sample window per tile (%d k-blocks) exceeds the stage capacity (%d)", stage_blocks, kTcMaxStageBlocks);
-    tc_plan_destroy(tp);
-    return nullptr;
+  if (stats[1] & 1) return refuse_free("a sample window of a voxel group needs more than 2 MMA passes (grid too coarse)");
+  if (stats[1] & 2) {
+    *retry_narrow = groups > 1 && !(stats[1] & 1);
+    return refuse_free("the sample windows of a tile's voxel groups do not fit one staged box (grid too coarse)");
   }
+  if (stats[1] & 4) return refuse_free("internal: window start out of range");
 
   // Tile order: depth slab by depth slab (heaviest slab first), all lateral tiles of a slab side by
   // side.  The CTAs of a wave then walk the same receivers of the same depth at about the same
@@ -208,58 +224,104 @@ TcPlan* tc_plan_create(const Params& P, const das_plan_desc_t& d, int n_frames, 
   }
   if ((e = up(tp, tiles_s, &dv.tiles)) != cudaSuccess || (e = up(tp, tbase_s, &dv.tbase)) != cudaSuccess) return fail(e);
 
-  dv.stage_blocks = stage_blocks;
-  // A ring: as deep as tensor memory allows next to the accumulators (512 columns: kTcG * 2 Bc of D)
-  dv.a_shift = 3;
-  if (const char* ev = getenv("DAS_TC_ABUFS")) dv.a_shift = std::min(3, std::max(0, atoi(ev)));   // tuning sweeps only
-  while (dv.a_shift > 0 && kTcG * 2 * Bc + kTcG * (1 << dv.a_shift) * kTcACols > kTcTmemCols) --dv.a_shift;
-  dv.a_bufs = 1 << dv.a_shift;
-  // Stage ring: `qs` window slots per stage (the fewer barrier rounds the better: the producer and
-  // the MMA issuers are serial latency chains) and as many stages as cover the L2 latency of a
-  // window.  Measured at the headline: (qs, stages) = (8, 2) 94 ms, (4, 4) 96 ms, (1, 6) 111 ms.
-  dv.qs = 8;
-  dv.n_stages = 2;
-  while (dv.qs > 1 && tc_smem_bytes(Bc, stage_blocks, dv.qs, 2) > 200 * 1024) dv.qs /= 2;
-  if (const char* ev = getenv("DAS_TC_QS")) dv.qs = std::min(16, std::max(1, atoi(ev)));                               // tuning sweeps only
+  static_assert(kTcG * 2 * 64 + kTcG * kTcABufs * kTcACols <= kTcTmemCols, "accumulators + A slots exceed tensor memory");
+  // Stage ring: `qs` boxes (consecutive transmits of one receiver) per stage, one barrier round per qs items
+  // (the producer and the MMA issuers are serial latency chains), and as many stages as shared memory holds
+  // (boxes in flight = what covers the L2 / HBM latency of the TMA copies).
+  dv.qs = std::min(8, Q);
+  if (const char* ev = getenv("DAS_TC_QS")) dv.qs = std::min(kTcMaxQs, std::max(1, atoi(ev)));                          // tuning sweeps only
+  while (dv.qs > 1 && tc_smem_bytes(Bc, dv.qs, kTcMinStages) > 200 * 1024) dv.qs /= 2;
+  dv.n_stages = kTcMinStages;
+  while (dv.n_stages < 6 && tc_smem_bytes(Bc, dv.qs, dv.n_stages + 1) <= 200 * 1024) ++dv.n_stages;
   if (const char* ev = getenv("DAS_TC_STAGES")) dv.n_stages = std::min(kTcMaxStages, std::max(kTcMinStages, atoi(ev)));   // tuning sweeps only
-  else while (dv.n_stages < 4 && dv.qs * dv.n_stages < 8 && tc_smem_bytes(Bc, stage_blocks, dv.qs, dv.n_stages + 1) <= 200 * 1024) ++dv.n_stages;
-  while (dv.n_stages > kTcMinStages && tc_smem_bytes(Bc, stage_blocks, dv.qs, dv.n_stages) > 200 * 1024) --dv.n_stages;
-  tp->smem = tc_smem_bytes(Bc, stage_blocks, dv.qs, dv.n_stages);
+  while (dv.n_stages > kTcMinStages && tc_smem_bytes(Bc, dv.qs, dv.n_stages) > 200 * 1024) --dv.n_stages;
+  tp->smem = tc_smem_bytes(Bc, dv.qs, dv.n_stages);
   if (tp->smem > 200 * 1024) return refuse_free("stage ring does not fit in shared memory");
   tp->grid = std::max(1, std::min(n_tiles * dv.n_chunks, prop.multiProcessorCount));
   return tp;
 }
 
+// The TMA descriptor of the converted data (caller-owned buffer, so it is encoded per launch: a host-side
+// table fill, no driver call into the device).  3-D tensor of FP16:
+//   dim 0: one column group's record, 2 K rows (16 bytes each) per sample, contiguous
+//   dim 1: the N / 8 column groups of a record      dim 2: the records (chunk, m, q)
+// box = (2 box_samples K rows, N / 8, 1): lands in shared memory as [column group][K row][8 columns], the
+// MN-major no-swizzle operand layout of tcgen05.mma with SBO = (K rows of the box) * 16 bytes.  Out-of-range K rows (before
+// sample 0, beyond sample K - 1) are filled with zeros by the TMA unit: no padding in memory.
+namespace {
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+cudaError_t tc_encode_map(const TcPlan* tp, const Params& P, const void* d_conv, int box_samples, CUtensorMap* map) {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q);
+    if (e != cudaSuccess) return e;
+    if (!p || q != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
+    fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  const cuuint64_t J = (cuuint64_t)(2 * tp->dev.Bc / 8);
+  // elements are 32-bit words (the box's inner extent is limited to 256 ELEMENTS): 4 per K row
+  const cuuint64_t dims[3] = {8ull * (cuuint64_t)P.K, J, (cuuint64_t)tp->dev.n_chunks * P.M * P.Q};
+  const cuuint64_t strides[2] = {dims[0] * 4ull, dims[0] * 4ull * J};
+  const cuuint32_t box[3] = {8u * (cuuint32_t)box_samples, (cuuint32_t)J, 1u};
+  const cuuint32_t estr[3] = {1u, 1u, 1u};
+  const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_UINT32, 3, const_cast<void*>(d_conv), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+}  // namespace
+
 cudaError_t launch_tc(const TcPlan* tp, const Params& P, const void* d_conv, void* d_out, cudaStream_t s) {
   count_launch();
-  return launch_tc_kernel(tp->dev, P, d_conv, d_out, tp->grid, tp->smem, s);
+  alignas(64) CUtensorMap map[2];
+  cudaError_t me = tc_encode_map(tp, P, d_conv, kTcBoxSmall, &map[0]);
+  if (me == cudaSuccess) me = tc_encode_map(tp, P, d_conv, kTcBoxBig, &map[1]);
+  if (me != cudaSuccess) return me;
+#ifdef DAS_TC_PROF
+  // development aid: cycle accounting per warp role, printed after a synchronising launch
+  if (getenv("DAS_TC_PROF")) {
+    TcDev dv = tp->dev;
+    const size_t n = (size_t)tp->grid * 32 * 8;
+    cudaMalloc(&dv.prof, n * sizeof(unsigned long long));
+    cudaMemset(dv.prof, 0, n * sizeof(unsigned long long));
+    cudaError_t e = launch_tc_kernel(dv, P, map, d_out, tp->grid, tp->smem, s);
+    cudaStreamSynchronize(s);
+    std::vector<unsigned long long> h(n);
+    cudaMemcpy(h.data(), dv.prof, n * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+    cudaFree(dv.prof);
+    double acc[20][8] = {};
+    for (int c = 0; c < tp->grid; ++c) for (int w = 0; w < 20; ++w) for (int k = 0; k < 8; ++k) acc[w][k] += (double)h[((size_t)c * 32 + w) * 8 + k] / tp->grid;
+    for (int w = 0; w < 20; ++w)
+      fprintf(stderr, "[tc prof] warp %2d total %.3e  w1 %.3e w2 %.3e w3 %.3e w4 %.3e w5 %.3e w6 %.3e\n", w, acc[w][0], acc[w][1], acc[w][2], acc[w][3], acc[w][4], acc[w][5], acc[w][6]);
+    return e;
+  }
+#endif
+  return launch_tc_kernel(tp->dev, P, map, d_out, tp->grid, tp->smem, s);
 }
 
 // ---- batch-inner layout transform + cast (PAPER.md:149 permute to batch-inner, :194-200 FP16) ----
 //   in : raw   [B][Q][M][K] complex64, samples contiguous in k (the paper's input layout)
-//   out: convb [chunk][M][Q][KBp][N = 2 Bc][8] FP16; k-block kb holds samples 4 (kb - kTcPadBlocks) + u,
-//        u = 0..3; column 2 b: (re, im) of frame b per sample; column 2 b + 1: (im, -re) = -j y;
-//        zero outside 0 <= k < K.
+//   out: convb [chunk][M][Q][J = 2 Bc / 8][2 K][8] FP16.  Record (chunk, m, q), column group j (the frames
+//        4 j .. 4 j + 3 of the chunk), K row 2 k holds y_k of those frames as (re, im) pairs, K row 2 k + 1
+//        holds -j y_k = (im, -re): one real MMA then yields Re and Im of the complex product (das_tc.cuh).
+//        No padding: the TMA copies of tc_kernel fill the rows outside 0 <= k < K with zeros.
 // One CTA per (m, q, chunk): reads Bc rows of K samples (coalesced along k), transposes through
-// shared memory in pieces of 64 samples, writes 16-byte column entries (coalesced along columns).
+// shared memory in pieces of 64 samples, writes 32-byte row pairs (coalesced along k within a column group).
 namespace {
-constexpr int kCbSamples = 64;      // samples per piece = 16 k-blocks
+constexpr int kCbSamples = 64;      // samples per piece
 
 __global__ void __launch_bounds__(256)
-convert_batch_kernel(const float2* __restrict__ raw, uint4* __restrict__ convb, int M, int Q, int K, int KBp,
+convert_batch_kernel(const float2* __restrict__ raw, uint4* __restrict__ convb, int M, int Q, int K,
                      int Bc, int n_frames, float scale) {
   extern __shared__ __align__(16) unsigned char cb_smem[];
   unsigned* tile = reinterpret_cast<unsigned*>(cb_smem);          // [Bc][kCbSamples + 1] half2 (re, im)
   const int q = blockIdx.x % Q, m = (blockIdx.x / Q) % M, chunk = blockIdx.x / (Q * M);
-  const int N = 2 * Bc;
-  uint4* row = convb + (((long long)chunk * M + m) * Q + q) * (long long)KBp * N;
-  const uint4 zero4 = make_uint4(0u, 0u, 0u, 0u);
-  const int Kb = (K + kTcBlk - 1) / kTcBlk;
-  // zero pads
-  for (int i = threadIdx.x; i < kTcPadBlocks * N; i += blockDim.x) {
-    row[i] = zero4;
-    row[(long long)(kTcPadBlocks + Kb) * N + i] = zero4;
-  }
+  const int J = 2 * Bc / 8;
+  uint4* rec = convb + (((long long)chunk * M + m) * Q + q) * (long long)J * (2LL * K);
   for (int k0 = 0; k0 < K; k0 += kCbSamples) {
     __syncthreads();
     for (int i = threadIdx.x; i < Bc * kCbSamples; i += blockDim.x) {
@@ -273,17 +335,19 @@ convert_batch_kernel(const float2* __restrict__ raw, uint4* __restrict__ convb, 
       tile[b * (kCbSamples + 1) + kk] = v;
     }
     __syncthreads();
-    const int nblk = min(kCbSamples / kTcBlk, Kb - k0 / kTcBlk);
-    for (int i = threadIdx.x; i < nblk * N; i += blockDim.x) {
-      const int col = i % N, kb = i / N, b = col >> 1;
-      unsigned w[4];
+    const int nk = min(kCbSamples, K - k0);
+    for (int i = threadIdx.x; i < J * nk; i += blockDim.x) {
+      const int j = i / nk, kk = i % nk;
+      unsigned y[4], z[4];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const unsigned v = tile[b * (kCbSamples + 1) + kb * kTcBlk + u];        // (re, im)
-        // odd column: (im, -re): swap halves, flip the sign of the new high half
-        w[u] = (col & 1) ? (((v >> 16) | (v << 16)) ^ 0x80000000u) : v;
+      for (int f = 0; f < 4; ++f) {
+        const unsigned v = tile[(4 * j + f) * (kCbSamples + 1) + kk];             // (re, im)
+        y[f] = v;
+        z[f] = ((v >> 16) | (v << 16)) ^ 0x80000000u;                              // (im, -re): swap halves, flip the new high half
       }
-      row[(long long)(kTcPadBlocks + k0 / kTcBlk + kb) * N + col] = make_uint4(w[0], w[1], w[2], w[3]);
+      uint4* dst = rec + ((long long)j * (2LL * K) + 2LL * (k0 + kk));
+      dst[0] = make_uint4(y[0], y[1], y[2], y[3]);
+      dst[1] = make_uint4(z[0], z[1], z[2], z[3]);
     }
   }
 }
@@ -295,7 +359,7 @@ cudaError_t launch_convert_batch(const TcPlan* tp, const Params& P, const void* 
   const size_t smem = (size_t)dv.Bc * (kCbSamples + 1) * 4;
   const long long blocks = (long long)dv.n_chunks * P.M * P.Q;
   convert_batch_kernel<<<(unsigned)blocks, 256, smem, s>>>(static_cast<const float2*>(d_raw), static_cast<uint4*>(d_conv),
-                                                             P.M, P.Q, P.K, dv.KBp, dv.Bc, tp->n_frames, scale);
+                                                             P.M, P.Q, P.K, dv.Bc, tp->n_frames, scale);
   count_launch();
   return cudaGetLastError();
 }
