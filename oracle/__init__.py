@@ -19,6 +19,17 @@ from . import build as _build
 
 _lib = None
 
+WINDOWS = {"boxcar": 0, "hann": 1, "tukey": 2}
+INTERPS = {"linear": 0, "cubic": 1}
+
+
+class _Opts(ctypes.Structure):
+    """das_oracle_opts of das_oracle.c."""
+    _fields_ = [("tau_tx_tab", ctypes.POINTER(ctypes.c_float)), ("w_tx_tab", ctypes.POINTER(ctypes.c_float)),
+                ("obs_off", ctypes.POINTER(ctypes.c_longlong)), ("obs_q", ctypes.POINTER(ctypes.c_int)),
+                ("vox_pos", ctypes.POINTER(ctypes.c_float)), ("window", ctypes.c_int),
+                ("window_param", ctypes.c_float), ("interp", ctypes.c_int)]
+
 
 def _load():
     global _lib
@@ -35,6 +46,8 @@ def _load():
             ctypes.c_float, ctypes.c_float, ctypes.c_float, ctypes.c_float, ctypes.c_float,
             ctypes.c_int, ctypes.c_int, f32p, i64p, ctypes.c_longlong,
             f64p, i64p, f64p, f64p, ctypes.c_double]
+        lib.das_oracle_ex.restype = ctypes.c_int
+        lib.das_oracle_ex.argtypes = lib.das_oracle.argtypes + [ctypes.POINTER(_Opts)]
         lib.das_oracle_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -50,12 +63,18 @@ def _p(a, ty):
 
 
 def das(w, *, y=None, voxels: Optional[np.ndarray] = None, want_count=False, want_l1=False,
-        want_slack=False, slack_rel: float = 1e-6):
+        want_slack=False, slack_rel: float = 1e-6, tau_tx=None, w_tx=None, obs=None, vox_pos=None,
+        window: str = "boxcar", window_param: float = 0.5, interp: str = "linear"):
     """Oracle DAS of workload ``w`` (optionally with replacement channel data ``y``).
 
     Returns the full volume [nx,ny,nz] (complex128 for IQ, float64 for RF), or, when
     ``voxels`` (flat indices (ix*ny+iy)*nz+iz) is given, a 1-D array over those voxels.
-    With want_* flags returns a dict {"out", "count", "l1", "slack"}."""
+    With want_* flags returns a dict {"out", "count", "l1", "slack"}.
+
+    Options of the paper's general interface (das_oracle.c header): ``tau_tx`` / ``w_tx`` tables
+    [Q, N] (N = number of voxels, flat order), ``obs`` = (obs_off[N+1], obs_q[]) CSR observation
+    lists, ``vox_pos`` [N,3] an arbitrary voxel list (output then has shape [N,1,1]), ``window`` in
+    WINDOWS with the Tukey taper ``window_param``, ``interp`` in INTERPS."""
     lib = _load()
     y = w.y if y is None else y
     iq = int(w.data_kind) == 0
@@ -69,6 +88,28 @@ def das(w, *, y=None, voxels: Optional[np.ndarray] = None, want_count=False, wan
     tv = np.ascontiguousarray(w.tx_v, dtype=np.float32)
     t0 = np.ascontiguousarray(w.tx_t0, dtype=np.float32)
     xs, ys, zs = (np.ascontiguousarray(a, dtype=np.float32) for a in (w.xs, w.ys, w.zs))
+    opts = _Opts()
+    keep = []
+    if vox_pos is not None:
+        vp = np.ascontiguousarray(vox_pos, dtype=np.float32).reshape(-1, 3)
+        xs, ys, zs = np.zeros(len(vp), np.float32), np.zeros(1, np.float32), np.zeros(1, np.float32)
+        opts.vox_pos = _p(vp, ctypes.c_float)
+        keep.append(vp)
+    n_tot = len(xs) * len(ys) * len(zs)
+    for name, tab in (("tau_tx_tab", tau_tx), ("w_tx_tab", w_tx)):
+        if tab is not None:
+            t = np.ascontiguousarray(tab, dtype=np.float32).reshape(q_n, n_tot)
+            setattr(opts, name, _p(t, ctypes.c_float))
+            keep.append(t)
+    if obs is not None:
+        off = np.ascontiguousarray(obs[0], dtype=np.int64).reshape(-1)
+        oq = np.ascontiguousarray(obs[1], dtype=np.int32).reshape(-1)
+        if len(off) != n_tot + 1 or off[0] != 0 or off[-1] != len(oq) or np.any(np.diff(off) < 0):
+            raise ValueError("malformed observation lists")
+        oq = oq if len(oq) else np.zeros(1, np.int32)
+        opts.obs_off, opts.obs_q = _p(off, ctypes.c_longlong), _p(oq, ctypes.c_int)
+        keep += [off, oq]
+    opts.window, opts.window_param, opts.interp = WINDOWS[window], float(window_param), INTERPS[interp]
     if voxels is None:
         vox, n_eval = None, len(xs) * len(ys) * len(zs)
     else:
@@ -79,7 +120,7 @@ def das(w, *, y=None, voxels: Optional[np.ndarray] = None, want_count=False, wan
     l1 = np.zeros(n_eval, dtype=np.float64) if want_l1 else None
     slack = np.zeros(n_eval, dtype=np.float64) if want_slack else None
     yf = y.view(np.float32)
-    rc = lib.das_oracle(
+    rc = lib.das_oracle_ex(
         _p(elem, ctypes.c_float), _p(edir, ctypes.c_float), m_n,
         _p(ttype, ctypes.c_int), _p(tv, ctypes.c_float), _p(t0, ctypes.c_float), q_n,
         _p(xs, ctypes.c_float), len(xs), _p(ys, ctypes.c_float), len(ys), _p(zs, ctypes.c_float), len(zs),
@@ -87,7 +128,7 @@ def das(w, *, y=None, voxels: Optional[np.ndarray] = None, want_count=False, wan
         k_n, int(w.data_kind), _p(yf, ctypes.c_float),
         _p(vox, ctypes.c_longlong), n_eval,
         _p(out, ctypes.c_double), _p(cnt, ctypes.c_longlong), _p(l1, ctypes.c_double),
-        _p(slack, ctypes.c_double), float(slack_rel))
+        _p(slack, ctypes.c_double), float(slack_rel), ctypes.byref(opts))
     if rc != 0:
         raise ValueError("das_oracle rejected its arguments")
     res = out.view(np.complex128) if iq else out
