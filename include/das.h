@@ -51,6 +51,14 @@ typedef enum {
 typedef enum { DAS_TX_PLANE = 0, DAS_TX_DIVERGING = 1 } das_tx_type_t;
 typedef enum { DAS_DATA_IQ = 0, DAS_DATA_RF = 1 } das_data_kind_t;
 typedef enum { DAS_STORE_FP32 = 0, DAS_STORE_FP16 = 1 } das_storage_t;
+/* Receive window on the f-number cone ("receive weight ... origin and a direction"; DESIGN.md
+ * reading W1).  With u = 2 f# rho / a in [0, 1] the normalised radius inside the cone:
+ *   BOXCAR w_rx = 1 | HANN w_rx = (1 + cos(pi u)) / 2 | TUKEY(b) w_rx = 1 for u <= 1 - b,
+ *   (1 + cos(pi (u - 1 + b) / b)) / 2 beyond; 0 outside the cone; every window is 1 when f_number <= 0. */
+typedef enum { DAS_WINDOW_BOXCAR = 0, DAS_WINDOW_HANN = 1, DAS_WINDOW_TUKEY = 2 } das_window_t;
+/* Temporal interpolation: LINEAR is the paper's; CUBIC is the 4-tap cubic convolution
+ * (Keys, a = -1/2) on y[k-1..k+2], the term dropped unless 1 <= k <= K-3 (reading W2). */
+typedef enum { DAS_INTERP_LINEAR = 0, DAS_INTERP_CUBIC = 1 } das_interp_t;
 typedef enum {
   DAS_ALGO_AUTO = 0,     /* tiled kernel when the geometry allows it, else the general kernel */
   DAS_ALGO_GENERAL = 1,  /* one thread per voxel, any element positions / normals (Alg. 1 shape) */
@@ -90,8 +98,20 @@ typedef struct {
   int   device;       /* CUDA device ordinal */
   int   n_frames;     /* B, frames per call that share this geometry; 0 or 1 = one frame.
                          With B > 1 das_convert / das_execute / das_beamform_host take B frames:
-                         raw [B][Q][M][K], output [B][nx][ny][nz]; every frame is beamformed exactly
-                         as a one-frame call would (DAS_ALGO_TC, else frame by frame). */
+                         raw [B][Q][M][K], output [B][nx][ny][nz]; every frame is the sum Eq. 2 defines
+                         for it (DAS_ALGO_TC: weights rounded to FP16, else frame by frame). */
+  /* ---- the paper's general interface (Alg. 1 "Require"); zero / NULL = off.  All HOST
+   *      pointers, copied at plan creation.  N = nx*ny*nz, voxel order = output order. ---- */
+  const float* tau_tx;      /* [Q][N] transmit delays tau_tx_qn in seconds; when given they
+                               replace the delay models of tx[] (type / v / t0 are then ignored) */
+  const float* w_tx;        /* [Q][N] transmit weights w_tx_qn (magnitude of the transmit field) */
+  const long long* obs_off; /* [N+1] CSR offsets of the per-voxel observation lists: voxel n sums */
+  const int* obs_q;         /* [obs_off[N]] only over the transmits listed for it, each at most once */
+  const float* vox_pos;     /* [N][3] an arbitrary voxel list ("{p_n}") instead of the grid axes:
+                               set nx = N, ny = nz = 1; xs / ys / zs are ignored.  General kernel only. */
+  int   window;             /* das_window_t */
+  float window_param;       /* TUKEY: taper fraction b in (0, 1] */
+  int   interp;             /* das_interp_t; CUBIC: general kernel only, one frame per call */
 } das_plan_desc_t;
 
 /* Validates *desc, uploads geometry and small derived tables to desc->device, chooses launch

@@ -27,6 +27,8 @@ TX_PLANE, TX_DIVERGING = 0, 1
 DATA_IQ, DATA_RF = 0, 1
 STORE_FP32, STORE_FP16 = 0, 1
 ALGO_AUTO, ALGO_GENERAL, ALGO_TILED, ALGO_TC = 0, 1, 2, 3
+WINDOW_BOXCAR, WINDOW_HANN, WINDOW_TUKEY = 0, 1, 2
+INTERP_LINEAR, INTERP_CUBIC = 0, 1
 
 # every symbol include/das.h declares (checked against the header by tests/test_abi.py)
 EXPORTS = ("das_plan_create", "das_plan_destroy", "das_raw_bytes", "das_converted_bytes",
@@ -50,6 +52,10 @@ class PlanDesc(ctypes.Structure):
         ("t_start", ctypes.c_float), ("f_number", ctypes.c_float),
         ("n_samples", ctypes.c_int), ("data_kind", ctypes.c_int), ("storage", ctypes.c_int),
         ("algo", ctypes.c_int), ("device", ctypes.c_int), ("n_frames", ctypes.c_int),
+        ("tau_tx", ctypes.POINTER(ctypes.c_float)), ("w_tx", ctypes.POINTER(ctypes.c_float)),
+        ("obs_off", ctypes.POINTER(ctypes.c_longlong)), ("obs_q", ctypes.POINTER(ctypes.c_int)),
+        ("vox_pos", ctypes.POINTER(ctypes.c_float)),
+        ("window", ctypes.c_int), ("window_param", ctypes.c_float), ("interp", ctypes.c_int),
     ]
 
 
@@ -135,7 +141,8 @@ class Plan:
 
     def __init__(self, elem_pos, tx_type, tx_v, tx_t0, xs, ys, zs, *, c, fc, fs, t_start=0.0,
                  f_number=1.0, n_samples, data_kind=DATA_IQ, storage=STORE_FP32, algo=ALGO_AUTO,
-                 device=0, elem_dir=None, n_frames=0):
+                 device=0, elem_dir=None, n_frames=0, tau_tx=None, w_tx=None, obs=None, vox_pos=None,
+                 window=WINDOW_BOXCAR, window_param=0.5, interp=INTERP_LINEAR):
         lib = load()
         self._lib = lib
         self._h = ctypes.c_void_p()
@@ -143,6 +150,9 @@ class Plan:
         tx_v = _f32(tx_v, (-1, 3))
         tx_t0 = _f32(tx_t0, (-1,))
         tx_type = np.ascontiguousarray(tx_type, dtype=np.int32).reshape(-1)
+        if vox_pos is not None:
+            vox_pos = _f32(vox_pos, (-1, 3))
+            xs, ys, zs = np.zeros(len(vox_pos), np.float32), np.zeros(1, np.float32), np.zeros(1, np.float32)
         xs, ys, zs = _f32(xs, (-1,)), _f32(ys, (-1,)), _f32(zs, (-1,))
         edir = None if elem_dir is None else _f32(elem_dir, (-1, 3))
         txs = (Transmit * len(tx_type))()
@@ -161,6 +171,24 @@ class Plan:
         d.c, d.fc, d.fs, d.t_start, d.f_number = float(c), float(fc), float(fs), float(t_start), float(f_number)
         d.n_samples, d.data_kind, d.storage = int(n_samples), int(data_kind), int(storage)
         d.algo, d.device, d.n_frames = int(algo), int(device), int(n_frames)
+        n_vox = len(xs) * len(ys) * len(zs)
+        keep = []
+        if tau_tx is not None:
+            tau_tx = _f32(tau_tx, (len(tx_type), n_vox)); d.tau_tx = tau_tx.ctypes.data_as(fp); keep.append(tau_tx)
+        if w_tx is not None:
+            w_tx = _f32(w_tx, (len(tx_type), n_vox)); d.w_tx = w_tx.ctypes.data_as(fp); keep.append(w_tx)
+        if obs is not None:
+            off = np.ascontiguousarray(obs[0], dtype=np.int64).reshape(-1)
+            oq = np.ascontiguousarray(obs[1], dtype=np.int32).reshape(-1)
+            if len(off) != n_vox + 1 or int(off[-1]) != len(oq):
+                raise ValueError("malformed observation lists")
+            oq = oq if len(oq) else np.zeros(1, np.int32)
+            d.obs_off = off.ctypes.data_as(ctypes.POINTER(ctypes.c_longlong))
+            d.obs_q = oq.ctypes.data_as(ctypes.POINTER(ctypes.c_int))
+            keep += [off, oq]
+        if vox_pos is not None:
+            d.vox_pos = vox_pos.ctypes.data_as(fp); keep.append(vox_pos)
+        d.window, d.window_param, d.interp = int(window), float(window_param), int(interp)
         self.desc = d
         _check(lib.das_plan_create(ctypes.byref(d), ctypes.byref(self._h)))
         self.grid_shape = (len(xs), len(ys), len(zs))
@@ -168,12 +196,13 @@ class Plan:
         self.n_tx, self.n_elem, self.n_samples = len(tx_type), len(elem_pos), int(n_samples)
 
     @classmethod
-    def from_workload(cls, w, *, storage=STORE_FP32, algo=ALGO_AUTO, device=0, n_frames=0):
-        """Plan for a ``workloads.Workload``-shaped object (duck-typed)."""
+    def from_workload(cls, w, *, storage=STORE_FP32, algo=ALGO_AUTO, device=0, n_frames=0, **options):
+        """Plan for a ``workloads.Workload``-shaped object (duck-typed); ``options`` are the keyword
+        arguments of the paper's general interface (tau_tx, w_tx, obs, vox_pos, window, window_param, interp)."""
         return cls(w.elem_pos, w.tx_type, w.tx_v, w.tx_t0, w.xs, w.ys, w.zs, c=w.c, fc=w.fc, fs=w.fs,
                    t_start=w.t_start, f_number=w.f_number, n_samples=w.n_samples,
                    data_kind=w.data_kind, storage=storage, algo=algo, device=device,
-                   elem_dir=getattr(w, "elem_dir", None), n_frames=n_frames)
+                   elem_dir=getattr(w, "elem_dir", None), n_frames=n_frames, **options)
 
     # sizes -------------------------------------------------------------------------------
     @property

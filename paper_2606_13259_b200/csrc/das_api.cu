@@ -118,7 +118,7 @@ das_status_t das_plan_create(const das_plan_desc_t* d, das_plan_t** out_plan) {
   if (!out_plan) { set_err("out_plan is NULL"); return DAS_ERR_INVALID_ARG; }
   *out_plan = nullptr;
   if (!d) { set_err("desc is NULL"); return DAS_ERR_INVALID_ARG; }
-  if (!d->elem_pos || !d->tx || !d->xs || !d->ys || !d->zs) {
+  if (!d->elem_pos || !d->tx || (!d->vox_pos && (!d->xs || !d->ys || !d->zs))) {
     set_err("elem_pos, tx, xs, ys, zs must be non-NULL"); return DAS_ERR_INVALID_ARG;
   }
   if (d->n_elem < 1 || d->n_tx < 1 || d->nx < 1 || d->ny < 1 || d->nz < 1) {
@@ -142,10 +142,26 @@ das_status_t das_plan_create(const das_plan_desc_t* d, das_plan_t** out_plan) {
     }
   }
   if (d->data_kind == DAS_DATA_RF && d->fc != 0.f) { set_err("fc must be 0 for RF data (no phase rotation)"); return DAS_ERR_INVALID_ARG; }
-  if (!finite_all(d->elem_pos, 3LL * d->n_elem) || !finite_all(d->xs, d->nx) ||
-      !finite_all(d->ys, d->ny) || !finite_all(d->zs, d->nz) ||
-      (d->elem_dir && !finite_all(d->elem_dir, 3LL * d->n_elem))) {
+  if (d->window != DAS_WINDOW_BOXCAR && d->window != DAS_WINDOW_HANN && d->window != DAS_WINDOW_TUKEY) { set_err("unknown window %d", d->window); return DAS_ERR_UNSUPPORTED; }
+  if (d->window == DAS_WINDOW_TUKEY && !(d->window_param > 0.f && d->window_param <= 1.f)) { set_err("the Tukey taper must lie in (0, 1]"); return DAS_ERR_INVALID_ARG; }
+  if (d->interp != DAS_INTERP_LINEAR && d->interp != DAS_INTERP_CUBIC) { set_err("unknown interp %d", d->interp); return DAS_ERR_UNSUPPORTED; }
+  if (d->interp == DAS_INTERP_CUBIC && d->n_samples < 4) { set_err("cubic interpolation needs n_samples >= 4"); return DAS_ERR_INVALID_ARG; }
+  if (d->vox_pos && (d->ny != 1 || d->nz != 1)) { set_err("with a voxel list set nx = N, ny = nz = 1"); return DAS_ERR_INVALID_ARG; }
+  if ((d->obs_off != nullptr) != (d->obs_q != nullptr)) { set_err("obs_off and obs_q go together"); return DAS_ERR_INVALID_ARG; }
+  const bool general_only = d->vox_pos != nullptr || d->interp == DAS_INTERP_CUBIC;
+  if (general_only && (d->algo == DAS_ALGO_TILED || d->algo == DAS_ALGO_TC)) {
+    set_err("voxel lists and cubic interpolation run in the general kernel only"); return DAS_ERR_UNSUPPORTED;
+  }
+  if (!finite_all(d->elem_pos, 3LL * d->n_elem) || (!d->vox_pos && (!finite_all(d->xs, d->nx) ||
+      !finite_all(d->ys, d->ny) || !finite_all(d->zs, d->nz))) ||
+      (d->elem_dir && !finite_all(d->elem_dir, 3LL * d->n_elem)) || (d->vox_pos && !finite_all(d->vox_pos, 3LL * d->nx))) {
     set_err("non-finite geometry value"); return DAS_ERR_INVALID_ARG;
+  }
+  {
+    const long long NQ = (long long)d->nx * d->ny * d->nz * d->n_tx;
+    if ((d->tau_tx && !finite_all(d->tau_tx, NQ)) || (d->w_tx && !finite_all(d->w_tx, NQ))) {
+      set_err("non-finite value in a transmit table"); return DAS_ERR_INVALID_ARG;
+    }
   }
   for (int q = 0; q < d->n_tx; ++q) {
     const das_transmit_t& t = d->tx[q];
@@ -192,7 +208,38 @@ das_status_t das_plan_create(const das_plan_desc_t* d, das_plan_t** out_plan) {
   DeviceGuard g(d->device);
   if (!g.ok) { das_status_t s = cuda_fail(g.err, "selecting the CUDA device"); delete p; return s; }
 
-  std::vector<float> hx(d->xs, d->xs + d->nx), hy(d->ys, d->ys + d->ny), hz(d->zs, d->zs + d->nz);
+  std::vector<float> hx, hy, hz;
+  std::vector<float4> hv;
+  if (d->vox_pos) {
+    hx.assign(d->nx, 0.f); hy.assign(1, 0.f); hz.assign(1, 0.f);
+    hv.resize(d->nx);
+    for (int i = 0; i < d->nx; ++i) hv[i] = make_float4(d->vox_pos[3 * i], d->vox_pos[3 * i + 1], d->vox_pos[3 * i + 2], 0.f);
+  } else {
+    hx.assign(d->xs, d->xs + d->nx); hy.assign(d->ys, d->ys + d->ny); hz.assign(d->zs, d->zs + d->nz);
+  }
+  // transmit tables; the observation lists are folded into the weights as exact zeros, which
+  // the kernels skip: a voxel then sums over its listed transmits only
+  std::vector<float> hw;
+  if (d->obs_off) {
+    if (d->obs_off[0] != 0) { set_err("obs_off[0] must be 0"); delete p; return DAS_ERR_INVALID_ARG; }
+    hw.assign((size_t)N * d->n_tx, 0.f);
+    for (long long n = 0; n < N; ++n) {
+      if (d->obs_off[n + 1] < d->obs_off[n]) { set_err("obs_off is not non-decreasing"); delete p; return DAS_ERR_INVALID_ARG; }
+      for (long long i = d->obs_off[n]; i < d->obs_off[n + 1]; ++i) {
+        const int q = d->obs_q[i];
+        if (q < 0 || q >= d->n_tx) { set_err("obs_q[%lld] = %d is not a transmit index", i, q); delete p; return DAS_ERR_INVALID_ARG; }
+        float& w = hw[(size_t)q * N + n];
+        if (w != 0.f) { set_err("voxel %lld lists transmit %d twice", n, q); delete p; return DAS_ERR_INVALID_ARG; }
+        w = 1.f;
+      }
+    }
+    if (d->w_tx) for (size_t i = 0; i < hw.size(); ++i) hw[i] = hw[i] != 0.f ? d->w_tx[i] : 0.f;
+  } else if (d->w_tx) {
+    hw.assign(d->w_tx, d->w_tx + (size_t)N * d->n_tx);
+  }
+  std::vector<float> htau;
+  if (d->tau_tx) htau.assign(d->tau_tx, d->tau_tx + (size_t)N * d->n_tx);
+  P.window = d->window; P.interp = d->interp; P.taper = d->window == DAS_WINDOW_TUKEY ? d->window_param : 1.f;
   std::vector<float4> he(d->n_elem), hd;
   for (int m = 0; m < d->n_elem; ++m) he[m] = make_float4(d->elem_pos[3 * m], d->elem_pos[3 * m + 1], d->elem_pos[3 * m + 2], 0.f);
   if (d->elem_dir) {
@@ -209,7 +256,10 @@ das_status_t das_plan_create(const das_plan_desc_t* d, das_plan_t** out_plan) {
   if ((e = upload(p, hx, &P.xs)) != cudaSuccess || (e = upload(p, hy, &P.ys)) != cudaSuccess ||
       (e = upload(p, hz, &P.zs)) != cudaSuccess || (e = upload(p, he, &P.elem)) != cudaSuccess ||
       (e = upload(p, ht, &P.tx)) != cudaSuccess ||
-      (d->elem_dir && (e = upload(p, hd, &P.edir)) != cudaSuccess)) {
+      (d->elem_dir && (e = upload(p, hd, &P.edir)) != cudaSuccess) ||
+      (!hv.empty() && (e = upload(p, hv, &P.vox)) != cudaSuccess) ||
+      (!hw.empty() && (e = upload(p, hw, &P.wtx_tab)) != cudaSuccess) ||
+      (!htau.empty() && (e = upload(p, htau, &P.tau_tab)) != cudaSuccess)) {
     das_status_t s = (e == cudaErrorMemoryAllocation) ? DAS_ERR_ALLOC : DAS_ERR_CUDA;
     cuda_fail(e, "uploading plan tables");
     free_plan(p);
@@ -217,7 +267,7 @@ das_status_t das_plan_create(const das_plan_desc_t* d, das_plan_t** out_plan) {
   }
 
   p->algo = DAS_ALGO_GENERAL;
-  if (d->algo == DAS_ALGO_TC || (d->algo == DAS_ALGO_AUTO && p->frames > 1)) {
+  if (!general_only && (d->algo == DAS_ALGO_TC || (d->algo == DAS_ALGO_AUTO && p->frames > 1))) {
     char why[256] = "";
     cudaError_t ce = cudaSuccess;
     p->tc = tc_plan_create(P, *d, p->frames, d->device, why, sizeof(why), &ce);
@@ -234,7 +284,7 @@ das_status_t das_plan_create(const das_plan_desc_t* d, das_plan_t** out_plan) {
       return DAS_ERR_UNSUPPORTED;
     }
   }
-  if (p->algo != DAS_ALGO_TC && d->algo != DAS_ALGO_GENERAL) {
+  if (p->algo != DAS_ALGO_TC && d->algo != DAS_ALGO_GENERAL && !general_only) {
     char why[256] = "";
     cudaError_t ce = cudaSuccess;
     p->tiled = tiled_plan_create(P, *d, d->device, why, sizeof(why), &ce);

@@ -58,33 +58,32 @@ general_kernel(const Params P, const T* __restrict__ conv, void* __restrict__ ou
   const int iz = (int)(n % P.nz);
   const int iy = (int)((n / P.nz) % P.ny);
   const int ix = (int)(n / ((long long)P.nz * P.ny));
-  const double px = (double)P.xs[ix], py = (double)P.ys[iy], pz = (double)P.zs[iz];
+  double px, py, pz;
+  if (P.vox) { const float4 v = __ldg(&P.vox[n]); px = (double)v.x; py = (double)v.y; pz = (double)v.z; }
+  else { px = (double)P.xs[ix]; py = (double)P.ys[iy]; pz = (double)P.zs[iz]; }
   const double inv_c = 1.0 / P.c;
-  const double lim_hi = (double)(P.K - 2);
+  const bool cubic = P.interp == DAS_INTERP_CUBIC;
+  const double lim_lo = cubic ? 1.0 : 0.0, lim_hi = (double)(P.K - (cubic ? 3 : 2));
   // 4 f#^2, rounded as ((4 f#) f#), the order the definition is evaluated in
   const double four_f2 = __dmul_rn(__dmul_rn(4.0, P.fnum), P.fnum);
 
   float tot_re = 0.f, tot_im = 0.f;
   for (int q0 = 0; q0 < P.Q; q0 += kQc) {
     double tau_tx[kQc];
-    float acc_re[kQc], acc_im[kQc];
+    float acc_re[kQc], acc_im[kQc], wq[kQc];
 #pragma unroll
     for (int j = 0; j < kQc; ++j) {
       acc_re[j] = 0.f; acc_im[j] = 0.f;
       const int q = min(q0 + j, P.Q - 1);
-      const TxDev tx = P.tx[q];
-      if (tx.type == DAS_TX_PLANE) {
-        tau_tx[j] = (px * tx.vx + py * tx.vy + pz * tx.vz) * inv_c + tx.t0;
-      } else {
-        const double ax = px - tx.vx, ay = py - tx.vy, az = pz - tx.vz;
-        tau_tx[j] = sqrt(ax * ax + ay * ay + az * az) * inv_c + tx.t0;
-      }
+      tau_tx[j] = tx_tau(P, q, n, px, py, pz);
+      wq[j] = tx_weight(P, q, n);                 // 0: the voxel does not list this transmit
     }
     for (int m = 0; m < P.M; ++m) {
       const float4 e = __ldg(&P.elem[m]);
       const double dx = px - (double)e.x, dy = py - (double)e.y, dz = pz - (double)e.z;
       const double dx2 = __dmul_rn(dx, dx), dy2 = __dmul_rn(dy, dy), dz2 = __dmul_rn(dz, dz);
       const double dd = __dadd_rn(__dadd_rn(dx2, dy2), dz2);
+      float w_rx = 1.f;
       if (P.apod) {
         double a, rho2;
         if (P.has_dir) {
@@ -96,22 +95,44 @@ general_kernel(const Params P, const T* __restrict__ conv, void* __restrict__ ou
           a = dz;
           rho2 = __dadd_rn(dx2, dy2);
         }
-        if (!(a > 0.0 && __dmul_rn(four_f2, rho2) <= __dmul_rn(a, a))) continue;
+        const double lhs = __dmul_rn(four_f2, rho2), rhs = __dmul_rn(a, a);
+        if (!(a > 0.0 && lhs <= rhs)) continue;
+        if (P.window != DAS_WINDOW_BOXCAR) w_rx = rx_window(P.window, P.taper, (float)(lhs / rhs));
       }
       const double tau_rx = sqrt(dd) * inv_c;
       const T* rowm = conv + (long long)m * P.Q * P.Kp;
 #pragma unroll
       for (int j = 0; j < kQc; ++j) {
         if (q0 + j >= P.Q) break;
+        if (wq[j] == 0.f) continue;
         const double tau = tau_tx[j] + tau_rx;
         const double t = (tau - P.t_start) * P.fs;
         const double kf = floor(t);
-        if (!(kf >= 0.0 && kf <= lim_hi)) continue;
-        const float ah = (float)(t - kf) - 0.5f;             // y[t] = mid_k + (alpha - 1/2) slope_k
-        const EntryF en = Sample<T>::load(rowm + (long long)(q0 + j) * P.Kp + (kPadLeft + (int)kf));
-        const float s_re = fmaf(ah, en.slope_re, en.mid_re);
+        if (!(kf >= lim_lo && kf <= lim_hi)) continue;
+        const float wg = wq[j] * w_rx;
+        const T* ent = rowm + (long long)(q0 + j) * P.Kp + (kPadLeft + (int)kf);
+        float s_re, s_im = 0.f;
+        if (cubic) {
+          // cubic convolution (Keys, a = -1/2) on y[k-1..k+2], rebuilt from the entries k-1 and k+1:
+          // y_k = mid_k - slope_k / 2, y_k+1 = mid_k + slope_k / 2
+          const float al = (float)(t - kf), a2 = al * al, a3 = a2 * al;
+          const float c0 = -0.5f * a3 + a2 - 0.5f * al, c1 = 1.5f * a3 - 2.5f * a2 + 1.f;
+          const float c2 = -1.5f * a3 + 2.f * a2 + 0.5f * al, c3 = 0.5f * a3 - 0.5f * a2;
+          const EntryF lo = Sample<T>::load(ent - 1), hi = Sample<T>::load(ent + 1);
+          s_re = c0 * fmaf(-0.5f, lo.slope_re, lo.mid_re) + c1 * fmaf(0.5f, lo.slope_re, lo.mid_re) +
+                 c2 * fmaf(-0.5f, hi.slope_re, hi.mid_re) + c3 * fmaf(0.5f, hi.slope_re, hi.mid_re);
+          if (IQ)
+            s_im = c0 * fmaf(-0.5f, lo.slope_im, lo.mid_im) + c1 * fmaf(0.5f, lo.slope_im, lo.mid_im) +
+                   c2 * fmaf(-0.5f, hi.slope_im, hi.mid_im) + c3 * fmaf(0.5f, hi.slope_im, hi.mid_im);
+        } else {
+          const float ah = (float)(t - kf) - 0.5f;             // y[t] = mid_k + (alpha - 1/2) slope_k
+          const EntryF en = Sample<T>::load(ent);
+          s_re = fmaf(ah, en.slope_re, en.mid_re);
+          if (IQ) s_im = fmaf(ah, en.slope_im, en.mid_im);
+        }
+        s_re *= wg;
         if (IQ) {
-          const float s_im = fmaf(ah, en.slope_im, en.mid_im);
+          s_im *= wg;
           double cyc = P.fc * tau;
           cyc -= rint(cyc);                        // phase in cycles, reduced to [-1/2, 1/2] in FP64
           float sn, cs;
@@ -143,9 +164,12 @@ count_kernel(const Params P, unsigned long long* __restrict__ counters) {
     const int iz = (int)(n % P.nz);
     const int iy = (int)((n / P.nz) % P.ny);
     const int ix = (int)(n / ((long long)P.nz * P.ny));
-    const double px = (double)P.xs[ix], py = (double)P.ys[iy], pz = (double)P.zs[iz];
+    double px, py, pz;
+    if (P.vox) { const float4 v = __ldg(&P.vox[n]); px = (double)v.x; py = (double)v.y; pz = (double)v.z; }
+    else { px = (double)P.xs[ix]; py = (double)P.ys[iy]; pz = (double)P.zs[iz]; }
     const double inv_c = 1.0 / P.c;
-    const double lim_hi = (double)(P.K - 2);
+    const bool cubic = P.interp == DAS_INTERP_CUBIC;
+    const double lim_lo = cubic ? 1.0 : 0.0, lim_hi = (double)(P.K - (cubic ? 3 : 2));
     const double four_f2 = __dmul_rn(__dmul_rn(4.0, P.fnum), P.fnum);
     for (int m = 0; m < P.M; ++m) {
       const float4 e = __ldg(&P.elem[m]);
@@ -168,16 +192,9 @@ count_kernel(const Params P, unsigned long long* __restrict__ counters) {
       ++pairs;
       const double tau_rx = sqrt(dd) * inv_c;
       for (int q = 0; q < P.Q; ++q) {
-        const TxDev tx = P.tx[q];
-        double tau_tx;
-        if (tx.type == DAS_TX_PLANE) {
-          tau_tx = (px * tx.vx + py * tx.vy + pz * tx.vz) * inv_c + tx.t0;
-        } else {
-          const double ax = px - tx.vx, ay = py - tx.vy, az = pz - tx.vz;
-          tau_tx = sqrt(ax * ax + ay * ay + az * az) * inv_c + tx.t0;
-        }
-        const double kf = floor((tau_tx + tau_rx - P.t_start) * P.fs);
-        if (kf >= 0.0 && kf <= lim_hi) ++terms;
+        if (tx_weight(P, q, n) == 0.f) continue;                // not on the voxel's observation list
+        const double kf = floor((tx_tau(P, q, n, px, py, pz) + tau_rx - P.t_start) * P.fs);
+        if (kf >= lim_lo && kf <= lim_hi) ++terms;
       }
     }
   }

@@ -53,7 +53,35 @@ struct Params {
   const float4* edir;   // [M] (nx, ny, nz, 0) or nullptr
   const TxDev* tx;      // [Q]
   double c, fc, fs, t_start, fnum;
+  // the paper's general interface (include/das.h); nullptr / 0 = off
+  const float* tau_tab;       // [Q][N] transmit delays in seconds
+  const float* wtx_tab;       // [Q][N] transmit weights with the observation lists folded in: 0 for a transmit a
+                              // voxel does not list (such terms are skipped, not multiplied)
+  const float4* vox;          // [N] voxel list (x, y, z, 0)
+  int window;                 // das_window_t
+  int interp;                 // das_interp_t
+  float taper;                // Tukey taper fraction
 };
+
+// Transmit delay of (q, voxel n at (x, y, z)) in seconds, FP64: the table when the plan has one, else the
+// delay model of the transmit (fn. 2, readings A1 / A2).
+__device__ __forceinline__ double tx_tau(const Params& P, int q, long long n, double x, double y, double z) {
+  if (P.tau_tab) return (double)__ldg(&P.tau_tab[(long long)q * ((long long)P.nx * P.ny * P.nz) + n]);
+  const TxDev tx = P.tx[q];
+  if (tx.type == DAS_TX_PLANE) return (x * tx.vx + y * tx.vy + z * tx.vz) / P.c + tx.t0;
+  const double bx = x - tx.vx, by = y - tx.vy, bz = z - tx.vz;
+  return sqrt(bx * bx + by * by + bz * bz) / P.c + tx.t0;
+}
+__device__ __forceinline__ float tx_weight(const Params& P, int q, long long n) {
+  return P.wtx_tab ? __ldg(&P.wtx_tab[(long long)q * ((long long)P.nx * P.ny * P.nz) + n]) : 1.f;
+}
+// Receive window on the f-number cone as a function of u^2 = 4 f#^2 rho^2 / a^2 (u in [0, 1] inside the cone)
+__device__ __forceinline__ float rx_window(int window, float taper, float u2) {
+  if (window == DAS_WINDOW_BOXCAR) return 1.f;
+  const float u = sqrtf(fminf(fmaxf(u2, 0.f), 1.f));
+  if (window == DAS_WINDOW_HANN) return 0.5f + 0.5f * cospif(u);
+  return u <= 1.f - taper ? 1.f : 0.5f + 0.5f * cospif((u - 1.f + taper) / taper);
+}
 
 // ---- kernels' host-side launchers (each returns the cudaError_t of its launch) -------------
 cudaError_t launch_convert(const Params& P, const void* d_raw, void* d_conv, float scale,

@@ -468,35 +468,39 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
         double cyc = tp.phase0 + tp.ratio * T;
         cyc -= rint(cyc);
         const float ang = 6.283185307179586f * (float)cyc;
-        if (j & 1) { Tf[j >> 1].y = tf; pc[j >> 1].y = cos_approx(ang); ps[j >> 1].y = sin_approx(ang); }
-        else       { Tf[j >> 1].x = tf; pc[j >> 1].x = cos_approx(ang); ps[j >> 1].x = sin_approx(ang); }
+        const float wq = tx_weight(P, qq, vx.n);                  // transmit weight (1 without a table), carried by Ptx
+        if (j & 1) { Tf[j >> 1].y = tf; pc[j >> 1].y = wq * cos_approx(ang); ps[j >> 1].y = wq * sin_approx(ang); }
+        else       { Tf[j >> 1].x = tf; pc[j >> 1].x = wq * cos_approx(ang); ps[j >> 1].x = wq * sin_approx(ang); }
       }
 
       // the list entry one iteration ahead: header, the group's 16 window codes, receiver position
       uint2 hd_n = make_uint2(0u, 0u);
       uint4 cw0_n = make_uint4(0u, 0u, 0u, 0u), cw1_n = cw0_n;
-      float4 el_n = make_float4(0.f, 0.f, 0.f, 0.f);
+      float4 el_n = make_float4(0.f, 0.f, 0.f, 0.f), dir_n = make_float4(0.f, 0.f, 1.f, 0.f);
       if (td.list_cnt) {
         const uint4* cp = reinterpret_cast<const uint4*>(tp.codes + ((long long)td.list_off * kTcG + g) * 16);
         hd_n = __ldg(&tp.list[td.list_off]);
         cw0_n = __ldg(cp); cw1_n = __ldg(cp + 1);
         el_n = __ldg(&P.elem[hd_n.x]);
+        if (P.has_dir) dir_n = __ldg(&P.edir[hd_n.x]);
       }
       for (int li = 0; li < td.list_cnt; ++li) {
         const uint2 hd = hd_n;
         const uint4 cw0 = cw0_n, cw1 = cw1_n;
-        const float4 el = el_n;
+        const float4 el = el_n, dir = dir_n;
         if (li + 1 < td.list_cnt) {
           const long long e = td.list_off + li + 1;
           const uint4* cp = reinterpret_cast<const uint4*>(tp.codes + (e * kTcG + g) * 16);
           hd_n = __ldg(&tp.list[e]);
           cw0_n = __ldg(cp); cw1_n = __ldg(cp + 1);
           el_n = __ldg(&P.elem[hd_n.x]);
+          if (P.has_dir) dir_n = __ldg(&P.edir[hd_n.x]);
         }
         if (!((hd.y >> g) & 1u)) continue;                    // no voxel of this group sees receiver m
         // per-(m, n): aperture, excess path, receive phase (as in das_tiled.cuh)
         bool act;
-        const float ex = tc_excess(tp, P, vx, el, act);
+        float wrx;
+        const float ex = tc_excess(tp, P, vx, el, dir, act, wrx);
         if (!__any_sync(0xffffffffu, act)) {
           // no voxel of this WARP sees the receiver: 32 zero rows per item, no arithmetic
           if (q16) tc_gen_receiver<false, true, true>(Tf, pc, ps, 0.f, 0.f, 0.f, cw0, cw1, tb_l, P.Q, P.K, st);
@@ -506,7 +510,7 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
         float cyc = tp.ratio_f * ex;
         cyc -= rintf(cyc);
         const float ang = 6.283185307179586f * cyc;
-        const float pr = act ? cos_approx(ang) : 0.f, pi = act ? sin_approx(ang) : 0.f;
+        const float pr = act ? wrx * cos_approx(ang) : 0.f, pi = act ? wrx * sin_approx(ang) : 0.f;
         if (q16) {
           if (td.edge) tc_gen_receiver<true, false, true>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, st);
           else tc_gen_receiver<false, false, true>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, st);
@@ -595,8 +599,10 @@ tc_window_kernel(const TcDev tp, const Params P, uint2* __restrict__ list, unsig
     if (tid < kTcG * 16) { kmn[tid / 16][tid % 16] = INT_MAX; kmx[tid / 16][tid % 16] = INT_MIN; }
     __syncthreads();
     const float4 el = __ldg(&P.elem[list[e].x]);
+    const float4 dir = P.has_dir ? __ldg(&P.edir[list[e].x]) : make_float4(0.f, 0.f, 1.f, 0.f);
     bool act;
-    const float ex = tc_excess(tp, P, vx, el, act);
+    float wrx_unused;
+    const float ex = tc_excess(tp, P, vx, el, dir, act, wrx_unused);
 #pragma unroll
     for (int q = 0; q < 16; ++q) {
       if (q < P.Q) {

@@ -116,6 +116,7 @@ __host__ __device__ inline int code_start(unsigned c) { return (int)((c >> 2) & 
 struct TcVoxel {
   float x, y, z, a, a2, a2e, band;
   double a_d;
+  long long n;                 // flat voxel index (clamped into the grid): row of the transmit tables
   int ix, iy, iz, izc;
   bool in_grid;
 };
@@ -126,6 +127,7 @@ __device__ __forceinline__ TcVoxel tc_voxel(const TcDev& tp, const Params& P, co
   v.in_grid = v.ix < P.nx && v.iy < P.ny && v.iz < P.nz && g < tp.groups;
   v.izc = min(v.iz, P.nz - 1);
   v.x = P.xs[min(v.ix, P.nx - 1)]; v.y = P.ys[min(v.iy, P.ny - 1)]; v.z = P.zs[v.izc];
+  v.n = ((long long)min(v.ix, P.nx - 1) * P.ny + min(v.iy, P.ny - 1)) * P.nz + v.izc;
   v.a_d = (double)v.z - tp.z_array;
   v.a = (float)v.a_d;
   v.a2 = v.a * v.a;
@@ -135,15 +137,23 @@ __device__ __forceinline__ TcVoxel tc_voxel(const TcDev& tp, const Params& P, co
 }
 // the part of the sample coordinate common to all receivers: T_q(n) = (tau_tx + a / c - t_start) fs, FP64
 __device__ __forceinline__ double tc_T(const Params& P, const TcVoxel& v, int q) {
-  return (tx_delay(P.tx[q], v.x, v.y, v.z, P.c) + v.a_d / P.c - P.t_start) * P.fs;
+  return (tx_tau(P, q, v.n, v.x, v.y, v.z) + v.a_d / P.c - P.t_start) * P.fs;
 }
 // receive excess path e_m(n) in samples (FP32) and the exactly classified aperture weight
-__device__ __forceinline__ float tc_excess(const TcDev& tp, const Params& P, const TcVoxel& v, float4 el, bool& act) {
+__device__ __forceinline__ float tc_excess(const TcDev& tp, const Params& P, const TcVoxel& v, float4 el, float4 dir, bool& act, float& wrx) {
   const float dx = v.x - el.x, dy = v.y - el.y;
   const float rho2 = fmaf(dx, dx, dy * dy);
-  const float lhs = tp.four_f2 * rho2;
-  act = lhs <= v.a2e;
-  if (fabsf(lhs - v.a2e) <= v.band) act = aperture_exact(v.x, v.y, el.x, el.y, P.zs, v.izc, tp.z_array, P.fnum);
+  float u2;
+  if (P.has_dir && P.apod) {
+    // tilted normal (coplanar positions): the delays are the planar array's, only the cone turns
+    act = aperture_dir(v.x, v.y, el.x, el.y, dx, dy, v.a, rho2, v.a2, dir, tp.four_f2, v.in_grid, P.zs, v.izc, tp.z_array, P.fnum, u2);
+  } else {
+    const float lhs = tp.four_f2 * rho2;
+    u2 = lhs * rcp_approx(v.a2);
+    act = lhs <= v.a2e;
+    if (fabsf(lhs - v.a2e) <= v.band) act = aperture_exact(v.x, v.y, el.x, el.y, P.zs, v.izc, tp.z_array, P.fnum);
+  }
+  wrx = (P.window != DAS_WINDOW_BOXCAR && P.apod) ? rx_window(P.window, P.taper, u2) : 1.f;   // receive window
   const float s2 = rho2 + v.a2;
   const float d = s2 * rsqrt_approx(s2);
   return (rho2 * tp.kappa_f) * rcp_approx(v.a + d);

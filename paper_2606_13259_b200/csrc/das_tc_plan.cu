@@ -69,6 +69,7 @@ static TcPlan* tc_plan_create_groups(const Params& P, const das_plan_desc_t& d, 
   auto refuse = [&](const char* msg) -> TcPlan* { snprintf(why, why_len, "%s", msg); return nullptr; };
   // ---- applicability ------------------------------------------------------------------------
   if (!P.iq || !P.fp16) return refuse("the tensor-core path needs IQ data in fp16 storage");
+  if (d.interp != DAS_INTERP_LINEAR || d.vox_pos) return refuse("voxel lists / cubic interpolation run in the general kernel");
   if (d.n_tx > 16) return refuse("more than 16 transmits");
   if (d.n_samples < 2 * kTcBoxBig) return refuse("fewer samples per trace than two staged boxes");
   if (n_frames < 8 || n_frames % 8) return refuse("frame count is not a multiple of 8");
@@ -77,10 +78,7 @@ static TcPlan* tc_plan_create_groups(const Params& P, const das_plan_desc_t& d, 
   const double z_a = d.elem_pos[2];
   for (int m = 0; m < d.n_elem; ++m)
     if ((double)d.elem_pos[3 * m + 2] != z_a) return refuse("receivers are not in one plane z = const");
-  if (d.elem_dir)
-    for (int m = 0; m < d.n_elem; ++m)
-      if (d.elem_dir[3 * m] != 0.f || d.elem_dir[3 * m + 1] != 0.f || d.elem_dir[3 * m + 2] != 1.f)
-        return refuse("receiver normals are not all (0,0,1)");
+  // tilted normals (elem_dir) are fine as long as the positions are coplanar: only the cone turns with the normal
   for (int i = 0; i < d.nz; ++i)
     if (!((double)d.zs[i] > z_a)) return refuse("a voxel plane is not in front of the array (z <= z_array)");
 
@@ -123,7 +121,8 @@ static TcPlan* tc_plan_create_groups(const Params& P, const das_plan_desc_t& d, 
               for (int j = td.iy0; j < iy1; ++j) {
                 const double x = d.xs[i], y = d.ys[j];
                 double tau;
-                if (tx.type == DAS_TX_PLANE) tau = (x * tx.v[0] + y * tx.v[1] + z * tx.v[2]) / c + tx.t0;
+                if (d.tau_tx) tau = d.tau_tx[(size_t)q * d.nx * d.ny * d.nz + ((size_t)i * d.ny + j) * d.nz + k];
+                else if (tx.type == DAS_TX_PLANE) tau = (x * tx.v[0] + y * tx.v[1] + z * tx.v[2]) / c + tx.t0;
                 else tau = std::sqrt((x - tx.v[0]) * (x - tx.v[0]) + (y - tx.v[1]) * (y - tx.v[1]) + (z - tx.v[2]) * (z - tx.v[2])) / c + tx.t0;
                 lo = std::min(lo, (tau + a / c - t_start) * fs);
               }
@@ -140,7 +139,18 @@ static TcPlan* tc_plan_create_groups(const Params& P, const das_plan_desc_t& d, 
           const double ex = d.elem_pos[3 * m], ey = d.elem_pos[3 * m + 1];
           const double nx_ = std::max(std::max(xlo - ex, ex - xhi), 0.0), ny_ = std::max(std::max(ylo - ey, ey - yhi), 0.0);
           const double rho_min = std::sqrt(nx_ * nx_ + ny_ * ny_);
-          if (apod && rho_min > cone * a_far * (1.0 + 1e-5)) continue;
+          if (apod && d.elem_dir) {
+            // tilted cone: bounding-sphere test of the angle between (p - e) and the normal (das_tiled_plan.cu)
+            double zlo = 1e300, zhi = -1e300;
+            for (int k = td.iz0; k < iz1; ++k) { zlo = std::min(zlo, (double)d.zs[k]); zhi = std::max(zhi, (double)d.zs[k]); }
+            const double cx = 0.5 * (xlo + xhi) - ex, cy = 0.5 * (ylo + yhi) - ey, cz = 0.5 * (zlo + zhi) - z_a;
+            const double R = 0.5 * std::sqrt((xhi - xlo) * (xhi - xlo) + (yhi - ylo) * (yhi - ylo) + (zhi - zlo) * (zhi - zlo));
+            const double dc = std::sqrt(cx * cx + cy * cy + cz * cz);
+            if (dc > R) {
+              const double ang = std::acos(std::max(-1.0, std::min(1.0, (cx * d.elem_dir[3 * m] + cy * d.elem_dir[3 * m + 1] + cz * d.elem_dir[3 * m + 2]) / dc)));
+              if (ang - std::asin(R / dc) > std::atan(cone) * (1.0 + 1e-5) + 1e-7) continue;
+            }
+          } else if (apod && rho_min > cone * a_far * (1.0 + 1e-5)) continue;
           list.push_back(make_uint2((unsigned)m, 0u));
         }
         td.list_cnt = (int)list.size() - td.list_off;

@@ -153,6 +153,8 @@ struct alignas(128) TiledSmem {
   float cyc[ModeTraits<MODE>::iq ? QC : 1][kConsumerThreads];   // transmit phase (cycles) per (q, voxel)
   float4 meta_raw[kRawStages];          // (ex, ey, E0, -) of the staged receiver
   float4 meta_tab[kTabStages];          // (ex, ey, E0, MAGIC + first entry of the stage)
+  float4 dir_raw[kRawStages];           // its normal (plans with elem_dir only)
+  float4 dir_tab[kTabStages];
   unsigned long long raw_full[kRawStages], raw_empty[kRawStages];
   unsigned long long tab_full[kTabStages], tab_empty[kTabStages];
 };
@@ -160,7 +162,7 @@ struct alignas(128) TiledSmem {
 // upper bound of sizeof(TiledSmem<QC, W, MODE>) for the plan's occupancy estimate
 __host__ __device__ inline size_t tiled_smem_bytes(int QC, int W, int iq, int fp16) {
   const size_t tb = iq ? 16 : 8, eb = (size_t)entry_bytes(iq, fp16);
-  return (size_t)QC * W * (kTabStages * tb + kRawStages * eb) + (size_t)(iq ? QC : 1) * kConsumerThreads * 4 + 512;
+  return (size_t)QC * W * (kTabStages * tb + kRawStages * eb) + (size_t)(iq ? QC : 1) * kConsumerThreads * 4 + 768;
 }
 
 // exact (definition-order, FP64) aperture test for pairs inside the FP32 guard band
@@ -172,6 +174,34 @@ static __device__ __noinline__ bool aperture_exact(float x, float y, float ex, f
   return __dmul_rn(four_f2, rho2) <= __dmul_rn(a, a);
 }
 
+// the same for a receiver with normal (nx, ny, nz): a = d.n, rho^2 = d.d - a^2, in the expression order of the
+// general kernel and of the definition
+static __device__ __noinline__ bool aperture_exact_dir(float x, float y, float ex, float ey, const float* zs, int iz, double z_array,
+                                                       double fnum, float nx, float ny, float nz) {
+  const double dz = (double)__ldg(&zs[iz]) - z_array;
+  const double dx = (double)x - (double)ex, dy = (double)y - (double)ey;
+  const double dd = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+  const double a = __dadd_rn(__dadd_rn(__dmul_rn(dx, (double)nx), __dmul_rn(dy, (double)ny)), __dmul_rn(dz, (double)nz));
+  const double rho2 = __dadd_rn(dd, -__dmul_rn(a, a));
+  const double four_f2 = __dmul_rn(__dmul_rn(4.0, fnum), fnum);
+  return a > 0.0 && __dmul_rn(four_f2, rho2) <= __dmul_rn(a, a);
+}
+// FP32 aperture test for a tilted normal with the exact test inside a guard band; u2 = 4 f#^2 rho^2 / a^2.
+// dx, dy: lateral offsets, az: depth above the array plane, rho2 = dx^2 + dy^2, a2 = az^2.
+__device__ __forceinline__ bool aperture_dir(float x, float y, float ex, float ey, float dx, float dy, float az, float rho2, float a2,
+                                             float4 dir, float four_f2, bool in_grid, const float* zs, int iz, double z_array,
+                                             double fnum, float& u2) {
+  const float an = fmaf(dx, dir.x, fmaf(dy, dir.y, az * dir.z));
+  const float dd = rho2 + a2, rhs = an * an;
+  const float lhs = four_f2 * (dd - rhs);
+  u2 = lhs * rcp_approx(fmaxf(rhs, 1e-30f));
+  bool act = in_grid && an > 0.f && lhs <= rhs;
+  // the cancellation in dd - an^2 and the sign test of an: both errors are a few ulp of dd
+  if (in_grid && (fabsf(lhs - rhs) <= 16.f * kBand * (four_f2 + 1.f) * dd || fabsf(an) <= 1e-5f * sqrtf(dd)))
+    act = aperture_exact_dir(x, y, ex, ey, zs, iz, z_array, fnum, dir.x, dir.y, dir.z);
+  return act;
+}
+
 __device__ __forceinline__ double tx_delay(const TxDev& tx, double x, double y, double z, double c) {
   if (tx.type == DAS_TX_PLANE) return (x * tx.vx + y * tx.vy + z * tx.vz) / c + tx.t0;
   const double bx = x - tx.vx, by = y - tx.vy, bz = z - tx.vz;
@@ -180,6 +210,7 @@ __device__ __forceinline__ double tx_delay(const TxDev& tx, double x, double y, 
 
 // Per-(receiver, voxel) geometry carried from one receiver-loop iteration to the next.
 struct Geo {
+  float u2;         // 4 f#^2 rho^2 / a^2: squared normalised radius inside the f-number cone (receive window)
   float rho2;       // lateral distance^2
   float ep;         // excess path e - E0 [samples]
   float mg;         // MAGIC + first table entry of the stage
@@ -201,15 +232,14 @@ __device__ __forceinline__ void term(unsigned a, float ts, float2 p1, float2 p2,
     acc = __ffma2_rn(make_float2(sv.y, sv.y), p2, acc);
   } else {
     const float2 v = lds64f<OFF>(a);                 // (c, slope)
-    acc.x += v.x;
-    acc.x = fmaf(ts, v.y, acc.x);
+    acc.x = fmaf(p1.x, fmaf(ts, v.y, v.x), acc.x);   // p1.x: the receive weight
   }
 }
 
 // Part 1: wait for the stage, read its meta entry, classify the aperture (exactly inside the
 // guard band).  a2e / band carry "voxel outside the grid" and "no apodization" (see the caller).
 __device__ __forceinline__ void geo_test(Geo& g, unsigned tab_full0, unsigned meta0, unsigned slot, unsigned phase,
-                                         float x, float y, int iz, float a2e, float band,
+                                         float x, float y, int iz, float a, float a2, float a2e, float band,
                                          const TiledDev& tp, const Params& P) {
   mbar_wait(tab_full0 + 8 * slot, phase);
   const float4 meta = lds128<0>(meta0 + 16 * slot);      // (ex, ey, E0, MAGIC + stage offset)
@@ -217,25 +247,34 @@ __device__ __forceinline__ void geo_test(Geo& g, unsigned tab_full0, unsigned me
   g.rho2 = fmaf(dx, dx, dy * dy);
   g.e0 = meta.z;
   g.mg = meta.w;
+  if (P.has_dir && P.apod) {
+    // tilted normal: the delays are those of the planar array, only the cone turns with the normal
+    const float4 dir = lds128<0>(meta0 + 16 * (kTabStages + kRawStages + slot));     // dir_tab[slot]
+    g.act = aperture_dir(x, y, meta.x, meta.y, dx, dy, a, g.rho2, a2, dir, tp.four_f2, a2e >= 0.f, P.zs, iz, tp.z_array, P.fnum, g.u2);
+    return;
+  }
   const float lhs = tp.four_f2 * g.rho2;
+  g.u2 = lhs * rcp_approx(a2);
   g.act = lhs <= a2e;
   if (fabsf(lhs - a2e) <= band) g.act = aperture_exact(x, y, meta.x, meta.y, P.zs, iz, tp.z_array, P.fnum);
 }
 // Part 2 (active lanes): excess path and receive phase.
 template <bool IQ>
-__device__ __forceinline__ void geo_finish(Geo& g, float a, float a2, const TiledDev& tp) {
+__device__ __forceinline__ void geo_finish(Geo& g, float a, float a2, const TiledDev& tp, const Params& P) {
   const float s2 = g.rho2 + a2;
   const float d = s2 * rsqrt_approx(s2);
   const float e = (g.rho2 * tp.kappa_f) * rcp_approx(a + d);
   g.ep = e - g.e0;
+  // receive window (include/das.h): the boxcar leaves the weight at 1
+  const float wrx = (P.window != DAS_WINDOW_BOXCAR && P.apod) ? rx_window(P.window, P.taper, g.u2) : 1.f;
   if (IQ) {
     float cyc = tp.ratio_f * e;
     cyc -= rintf(cyc);
     const float ang = 6.283185307179586f * cyc;
-    g.pr = cos_approx(ang);
-    g.pi = sin_approx(ang);
+    g.pr = wrx * cos_approx(ang);
+    g.pi = wrx * sin_approx(ang);
   } else {
-    g.pr = 1.f;
+    g.pr = wrx;
     g.pi = 0.f;
   }
 }
@@ -285,6 +324,7 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
             const float4 el = __ldg(&P.elem[m]);
             mbar_wait(raw_empty0 + 8 * slot, ((seq / kRawStages) & 1u) ^ 1u);
             if (lane == 0) {
+              if (P.has_dir) sm.dir_raw[slot] = __ldg(&P.edir[m]);
               sm.meta_raw[slot] = make_float4(el.x, el.y, (float)e0, 0.f);
               mbar_arrive_expect_tx(raw_full0 + 8 * slot, (unsigned)(nq * W * EB));
             }
@@ -312,6 +352,7 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
             float4 mt = sm.meta_raw[rs];
             mt.w = kMagic + (float)(ts * NE);
             sm.meta_tab[ts] = mt;
+            if (P.has_dir) sm.dir_tab[ts] = sm.dir_raw[rs];
           }
           const unsigned src = raw0 + rs * (NE * EB) + lane * EB, dst = tab0 + ts * (NE * TB) + lane * TB;
 #pragma unroll
@@ -365,6 +406,7 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
     const int izc = min(iz, P.nz - 1);
     const float x = P.xs[min(ix, P.nx - 1)], y = P.ys[min(iy, P.ny - 1)], z = P.zs[izc];
     const double a_d = (double)z - tp.z_array;
+    const long long n_flat = ((long long)min(ix, P.nx - 1) * P.ny + min(iy, P.ny - 1)) * P.nz + izc;   // voxel index (tables)
     // pin(): values the receiver loop reads every iteration are routed through a shuffle so that
     // ptxas keeps them in registers instead of rematerialising them (FP64 ops, select chains)
     const float a = pin((float)a_d);
@@ -383,7 +425,7 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
 #pragma unroll
       for (int j = 0; j < 2 * QP; ++j) {
         const int q = min(q0 + j, P.Q - 1);
-        const double T = (tx_delay(P.tx[q], x, y, z, P.c) + a_d / P.c - P.t_start) * P.fs;
+        const double T = (tx_tau(P, q, n_flat, x, y, z) + a_d / P.c - P.t_start) * P.fs;
         const int k0 = __ldg(&tp.k0tile[(long long)tile_i * P.Q + q]);
         const float tf = (float)(T - (double)k0 - 0.5);
         if (j & 1) Tf[j >> 1].y = tf; else Tf[j >> 1].x = tf;
@@ -398,9 +440,9 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
       // ---- receiver loop ---------------------------------------------------------------
       for (int li = 0; li < td.list_cnt; ++li) {
         Geo g;
-        geo_test(g, tab_full0, meta0, slot, phase, x, y, izc, a2e, band, tp, P);
+        geo_test(g, tab_full0, meta0, slot, phase, x, y, izc, a, a2, a2e, band, tp, P);
         if (g.act) {
-          geo_finish<IQ>(g, a, a2, tp);
+          geo_finish<IQ>(g, a, a2, tp, P);
           const float2 ep2 = make_float2(g.ep, g.ep), mg2 = make_float2(g.mg, g.mg);
           const float2 p1 = make_float2(g.pr, g.pi), p2 = make_float2(-g.pi, g.pr);
           constexpr int kRow = W * TB;
@@ -431,13 +473,14 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
 #pragma unroll
       for (int j = 0; j < 2 * QP; ++j) {
         if (j < QC && q0 + j < P.Q) {
+          const float wq = tx_weight(P, q0 + j, n_flat);        // transmit weight (1 without a table)
           if (IQ) {
             const float ang = 6.283185307179586f * sm.cyc[IQ ? j : 0][tid];
-            const float cs = cos_approx(ang), sn = sin_approx(ang);
+            const float cs = wq * cos_approx(ang), sn = wq * sin_approx(ang);
             out_re = fmaf(acc[j].x, cs, fmaf(-acc[j].y, sn, out_re));
             out_im = fmaf(acc[j].x, sn, fmaf(acc[j].y, cs, out_im));
           } else {
-            out_re += acc[j].x;
+            out_re = fmaf(wq, acc[j].x, out_re);
           }
         }
       }

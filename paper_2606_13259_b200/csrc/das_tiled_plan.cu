@@ -45,13 +45,12 @@ TiledPlan* tiled_plan_create(const Params& P, const das_plan_desc_t& d, int devi
   auto refuse = [&](const char* msg) -> TiledPlan* { snprintf(why, why_len, "%s", msg); return nullptr; };
   // ---- applicability ------------------------------------------------------------------------
   if (d.n_elem > 65535) return refuse("more than 65535 receivers");
+  if (d.interp != DAS_INTERP_LINEAR || d.vox_pos) return refuse("voxel lists / cubic interpolation run in the general kernel");
   const double z_a = d.elem_pos[2];
   for (int m = 0; m < d.n_elem; ++m)
     if ((double)d.elem_pos[3 * m + 2] != z_a) return refuse("receivers are not in one plane z = const");
-  if (d.elem_dir)
-    for (int m = 0; m < d.n_elem; ++m)
-      if (d.elem_dir[3 * m] != 0.f || d.elem_dir[3 * m + 1] != 0.f || d.elem_dir[3 * m + 2] != 1.f)
-        return refuse("receiver normals are not all (0,0,1)");
+  // tilted normals (elem_dir) are fine as long as the POSITIONS are coplanar: the delays are those of the
+  // planar array, only the f-number cone turns with the normal
   for (int i = 0; i < d.nz; ++i)
     if (!((double)d.zs[i] > z_a)) return refuse("a voxel plane is not in front of the array (z <= z_array)");
 
@@ -106,8 +105,19 @@ TiledPlan* tiled_plan_create(const Params& P, const das_plan_desc_t& d, int devi
             }
             lo = std::sqrt(dmin2); hi = std::sqrt(dmax2);
           }
-          const double t_lo = (lo / c + tx.t0 + a_lo / c - t_start) * fs;
-          const double t_hi = (hi / c + tx.t0 + a_hi / c - t_start) * fs;
+          double t_lo = (lo / c + tx.t0 + a_lo / c - t_start) * fs;
+          double t_hi = (hi / c + tx.t0 + a_hi / c - t_start) * fs;
+          if (d.tau_tx) {
+            // transmit delays from the table: exact bounds of T_q over the voxels of the tile
+            t_lo = 1e300; t_hi = -1e300;
+            for (int i = td.ix0; i < ix1; ++i)
+              for (int j = td.iy0; j < iy1; ++j)
+                for (int k = td.iz0; k < iz1; ++k) {
+                  const double tau = d.tau_tx[(size_t)q * d.nx * d.ny * d.nz + ((size_t)i * d.ny + j) * d.nz + k];
+                  const double T = (tau + ((double)d.zs[k] - z_a) / c - t_start) * fs;
+                  t_lo = std::min(t_lo, T); t_hi = std::max(t_hi, T);
+                }
+          }
           if (!(std::fabs(t_lo) < 1e9 && std::fabs(t_hi) < 1e9)) return refuse("sample coordinate out of int range");
           // Tf = T - k0 - 1/2 >= 1/2: the rounded entry index can never be negative
           const int k0 = floor_to_multiple((int)std::floor(t_lo) - 1, align);
@@ -123,9 +133,27 @@ TiledPlan* tiled_plan_create(const Params& P, const das_plan_desc_t& d, int devi
           const double nx_ = std::max(std::max(xlo - ex, ex - xhi), 0.0), ny_ = std::max(std::max(ylo - ey, ey - yhi), 0.0);
           const double fx = std::max(std::fabs(xlo - ex), std::fabs(xhi - ex)), fy = std::max(std::fabs(ylo - ey), std::fabs(yhi - ey));
           const double rho_min = std::sqrt(nx_ * nx_ + ny_ * ny_), rho_max = std::sqrt(fx * fx + fy * fy);
-          if (apod && rho_min > cone * a_hi * (1.0 + 1e-5)) continue;      // no voxel of the tile sees m
           double e_hi = excess(rho_max, a_lo);
-          if (apod) e_hi = std::min(e_hi, excess(cone * a_hi * (1.0 + 1e-5), a_hi));
+          if (apod && d.elem_dir) {
+            // tilted cone: a voxel is active iff the angle between (p - e) and the normal is <= atan(1 / (2 f#)).
+            // Over the tile that angle is at least angle(centre) - (angular radius of the tile's bounding sphere).
+            const double nv[3] = {d.elem_dir[3 * m], d.elem_dir[3 * m + 1], d.elem_dir[3 * m + 2]};
+            const double cx = 0.5 * (xlo + xhi) - ex, cy = 0.5 * (ylo + yhi) - ey, cz = 0.5 * (zlo + zhi) - z_a;
+            const double R = 0.5 * std::sqrt((xhi - xlo) * (xhi - xlo) + (yhi - ylo) * (yhi - ylo) + (zhi - zlo) * (zhi - zlo));
+            const double dc = std::sqrt(cx * cx + cy * cy + cz * cz);
+            const double theta_c = std::atan(cone);
+            if (dc > R) {
+              const double ang = std::acos(std::max(-1.0, std::min(1.0, (cx * nv[0] + cy * nv[1] + cz * nv[2]) / dc)));
+              if (ang - std::asin(R / dc) > theta_c * (1.0 + 1e-5) + 1e-7) continue;   // no voxel of the tile sees m
+            }
+            // lateral reach of the tilted cone at the deepest plane of the tile bounds the excess path
+            const double tilt = std::acos(std::max(-1.0, std::min(1.0, nv[2])));
+            const double reach = theta_c + tilt;
+            if (reach < 1.5) e_hi = std::min(e_hi, excess(std::tan(reach) * a_hi * (1.0 + 1e-5), a_hi));
+          } else if (apod) {
+            if (rho_min > cone * a_hi * (1.0 + 1e-5)) continue;             // no voxel of the tile sees m
+            e_hi = std::min(e_hi, excess(cone * a_hi * (1.0 + 1e-5), a_hi));
+          }
           const double e_lo = excess(rho_min, a_hi);
           const int e0 = floor_to_multiple(std::max((int)std::floor(e_lo * kappa), 0), align);
           if (e0 > 65535) return refuse("receive delay offset exceeds 16 bits");

@@ -295,22 +295,36 @@ def test_mixed_transmits_offset_array_nonzero_tstart(das_lib, algo):
     check(out, oracle.das(w), das_lib.STORE_FP32, das_lib, "mixed transmits")
 
 
-def test_tilted_normals_general_kernel(das_lib):
-    """Per-element normals: only the general kernel takes them; AUTO must fall back to it and
-    an explicit TILED request must be refused."""
+def test_tilted_normals(das_lib):
+    """Per-element normals.  With coplanar element POSITIONS the delays are the planar array's and only the
+    f-number cone turns, so the tiled kernel takes them too; a non-planar array goes to the general kernel
+    (AUTO falls back, an explicit TILED request is refused)."""
     import oracle
     das = das_lib
-    base = _cfg(1, (7, 6, 9))
+    base = _subgrid(1, slice(2, 30), slice(4, 25), slice(3, 28))
     rng = np.random.default_rng(3)
-    d = np.array([0, 0, 1.0]) + 0.25 * rng.normal(size=(64, 3))
+    d = np.array([0, 0, 1.0]) + 0.2 * rng.normal(size=(64, 3))
     d /= np.linalg.norm(d, axis=1, keepdims=True)
     w = wl.custom(base.elem_pos, base.tx_type, base.tx_v, base.tx_t0, base.xs, base.ys, base.zs,
                   fs=base.fs, n_samples=base.n_samples, f_number=0.9, y=base.y, elem_dir=d)
-    out, used = gpu_das(das, w, das.STORE_FP32, das.ALGO_AUTO)
+    ref = oracle.das(w)
+    for algo in (das.ALGO_GENERAL, das.ALGO_TILED):
+        for storage in (das.STORE_FP32, das.STORE_FP16):
+            out, used = gpu_das(das, w, storage, algo)
+            assert used == algo
+            check(out, ref, storage, das, f"tilted normals algo {algo}")
+    cnt_ref = oracle.das(w, want_count=True)["count"]
+    assert cnt_ref.min() < cnt_ref.max()                              # the cones do cut
+    # non-planar array: general kernel only
+    e2 = base.elem_pos.copy()
+    e2[:, 2] = (0.05e-3 * np.sin(np.arange(64))).astype(np.float32)
+    w2 = wl.custom(e2, base.tx_type, base.tx_v, base.tx_t0, base.xs, base.ys, base.zs,
+                   fs=base.fs, n_samples=base.n_samples, f_number=0.9, y=base.y, elem_dir=d)
+    out, used = gpu_das(das, w2, das.STORE_FP32, das.ALGO_AUTO)
     assert used == das.ALGO_GENERAL
-    check(out, oracle.das(w), das.STORE_FP32, das, "tilted normals")
+    check(out, oracle.das(w2), das.STORE_FP32, das, "non-planar array")
     with pytest.raises(das.DasError) as ei:
-        das.Plan.from_workload(w, algo=das.ALGO_TILED)
+        das.Plan.from_workload(w2, algo=das.ALGO_TILED)
     assert ei.value.status == das.ERR_UNSUPPORTED
 
 
