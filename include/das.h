@@ -50,7 +50,13 @@ typedef enum {
 
 typedef enum { DAS_TX_PLANE = 0, DAS_TX_DIVERGING = 1 } das_tx_type_t;
 typedef enum { DAS_DATA_IQ = 0, DAS_DATA_RF = 1 } das_data_kind_t;
-typedef enum { DAS_STORE_FP32 = 0, DAS_STORE_FP16 = 1 } das_storage_t;
+typedef enum {
+  DAS_STORE_FP32 = 0,
+  DAS_STORE_FP16 = 1,    /* the paper's mixed-precision storage */
+  DAS_STORE_FP8 = 2      /* e4m3, round to nearest even, saturating ("FP8 storage"): one frame per
+                            call, general and tiled kernels; the caller's `scale` must bring the data into the
+                            e4m3 range (|v| <= 448, resolution 2^-9 near zero); DESIGN.md gives the image quality */
+} das_storage_t;
 /* Receive window on the f-number cone ("receive weight ... origin and a direction"; DESIGN.md
  * reading W1).  With u = 2 f# rho / a in [0, 1] the normalised radius inside the cone:
  *   BOXCAR w_rx = 1 | HANN w_rx = (1 + cos(pi u)) / 2 | TUKEY(b) w_rx = 1 for u <= 1 - b,

@@ -101,3 +101,40 @@ def das(w, y=None, **opts) -> np.ndarray:
     else:
         x = x.reshape(len(w.xs), len(w.ys), len(w.zs))
     return x if int(w.data_kind) == 0 else x.real
+
+
+def das_from_interval_table(w, mid, slope) -> np.ndarray:
+    """The definition evaluated on a given table of sample INTERVALS: y[t] = mid_k + (alpha - 1/2) slope_k for
+    t = k + alpha (equal to linear interpolation, when mid_k = (y_k + y_k+1)/2 and
+    slope_k = y_k+1 - y_k).  ``mid`` / ``slope``: [Q, M, K-1].  Used to check a storage format that quantises
+    the interval table (fp8 storage) term by term instead of only statistically."""
+    e = np.asarray(w.elem_pos, dtype=np.float64)
+    gx, gy, gz = np.meshgrid(np.asarray(w.xs, np.float64), np.asarray(w.ys, np.float64),
+                             np.asarray(w.zs, np.float64), indexing="ij")
+    p = np.stack([gx.ravel(), gy.ravel(), gz.ravel()], axis=1)
+    c, fc, fs = (float(np.float32(v)) for v in (w.c, w.fc, w.fs))
+    t_start, fnum = float(np.float32(w.t_start)), float(np.float32(w.f_number))
+    k_n = int(w.n_samples)
+    d = p[:, None, :] - e[None, :, :]
+    dist = np.sqrt(np.einsum("nmi,nmi->nm", d, d))
+    if fnum > 0:
+        wrx = ((d[..., 2] > 0) & (4.0 * fnum * fnum * (d[..., 0] ** 2 + d[..., 1] ** 2) <= d[..., 2] ** 2)).astype(np.float64)
+    else:
+        wrx = np.ones_like(dist)
+    mid = np.asarray(mid).astype(np.complex128)
+    slope = np.asarray(slope).astype(np.complex128)
+    x = np.zeros(len(p), np.complex128)
+    mm = np.arange(len(e))[None, :]
+    for q in range(len(w.tx_type)):
+        v = np.asarray(w.tx_v[q], dtype=np.float64)
+        ttx = (p @ v / c if int(w.tx_type[q]) == 0 else np.linalg.norm(p - v, axis=1) / c) + float(w.tx_t0[q])
+        tau = ttx[:, None] + dist / c
+        t = (tau - t_start) * fs
+        k = np.floor(t)
+        ok = (k >= 0) & (k <= k_n - 2) & (wrx > 0)
+        ki = np.where(ok, k, 0).astype(np.int64)
+        s = mid[q][mm, ki] + (t - k - 0.5) * slope[q][mm, ki]
+        rot = np.exp(2j * np.pi * fc * tau) if int(w.data_kind) == 0 else 1.0
+        x += np.where(ok, s * rot, 0.0).sum(axis=1)
+    x = x.reshape(len(w.xs), len(w.ys), len(w.zs))
+    return x if int(w.data_kind) == 0 else x.real

@@ -25,7 +25,7 @@ from . import _build
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA, ERR_SIZE = range(6)
 TX_PLANE, TX_DIVERGING = 0, 1
 DATA_IQ, DATA_RF = 0, 1
-STORE_FP32, STORE_FP16 = 0, 1
+STORE_FP32, STORE_FP16, STORE_FP8 = 0, 1, 2
 ALGO_AUTO, ALGO_GENERAL, ALGO_TILED, ALGO_TC = 0, 1, 2, 3
 WINDOW_BOXCAR, WINDOW_HANN, WINDOW_TUKEY = 0, 1, 2
 INTERP_LINEAR, INTERP_CUBIC = 0, 1

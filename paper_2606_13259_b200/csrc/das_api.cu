@@ -131,7 +131,7 @@ das_status_t das_plan_create(const das_plan_desc_t* d, das_plan_t** out_plan) {
   if (!std::isfinite(d->t_start)) { set_err("t_start must be finite"); return DAS_ERR_INVALID_ARG; }
   if (!std::isfinite(d->f_number)) { set_err("f_number must be finite"); return DAS_ERR_INVALID_ARG; }
   if (d->data_kind != DAS_DATA_IQ && d->data_kind != DAS_DATA_RF) { set_err("unknown data_kind %d", d->data_kind); return DAS_ERR_UNSUPPORTED; }
-  if (d->storage != DAS_STORE_FP32 && d->storage != DAS_STORE_FP16) { set_err("unknown storage %d", d->storage); return DAS_ERR_UNSUPPORTED; }
+  if (d->storage != DAS_STORE_FP32 && d->storage != DAS_STORE_FP16 && d->storage != DAS_STORE_FP8) { set_err("unknown storage %d", d->storage); return DAS_ERR_UNSUPPORTED; }
   if (d->algo != DAS_ALGO_AUTO && d->algo != DAS_ALGO_GENERAL && d->algo != DAS_ALGO_TILED && d->algo != DAS_ALGO_TC) { set_err("unknown algo %d", d->algo); return DAS_ERR_UNSUPPORTED; }
   if (d->n_frames < 0 || d->n_frames > 4096) { set_err("n_frames = %d is outside [0, 4096]", d->n_frames); return DAS_ERR_INVALID_ARG; }
   if (d->algo == DAS_ALGO_TC) {
@@ -192,11 +192,12 @@ das_status_t das_plan_create(const das_plan_desc_t* d, das_plan_t** out_plan) {
   P.nx = d->nx; P.ny = d->ny; P.nz = d->nz;
   P.iq = d->data_kind == DAS_DATA_IQ;
   P.fp16 = d->storage == DAS_STORE_FP16;
+  P.fp8 = d->storage == DAS_STORE_FP8;
   P.apod = d->f_number > 0.f;
   P.has_dir = d->elem_dir != nullptr;
   P.c = d->c; P.fc = d->fc; P.fs = d->fs; P.t_start = d->t_start; P.fnum = d->f_number;
   const size_t in_elem = P.iq ? 8 : 4;
-  const size_t st_elem = (P.iq ? 2 : 1) * 2 * (P.fp16 ? 2 : 4);   // (mid, slope) entry
+  const size_t st_elem = (P.iq ? 2 : 1) * 2 * (P.fp8 ? 1 : (P.fp16 ? 2 : 4));   // (mid, slope) entry
   p->frames = d->n_frames > 1 ? d->n_frames : 1;
   p->raw1 = (size_t)rows * P.K * in_elem;
   p->conv1 = (size_t)rows * Kp * st_elem;

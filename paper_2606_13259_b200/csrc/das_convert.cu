@@ -48,17 +48,20 @@ __device__ __forceinline__ void make_entry(float4& e, float2 a, float2 b) {
 __device__ __forceinline__ void make_entry(uint2& e, float2 a, float2 b) {
   e = make_uint2(pack_h2(mid_of(a.x, b.x), mid_of(a.y, b.y)), pack_h2(slope_of(a.x, b.x), slope_of(a.y, b.y)));
 }
+__device__ __forceinline__ void make_entry(Fp8x4& e, float2 a, float2 b) {
+  e.v = (unsigned)float2_to_fp8x2(mid_of(a.x, b.x), mid_of(a.y, b.y)) | ((unsigned)float2_to_fp8x2(slope_of(a.x, b.x), slope_of(a.y, b.y)) << 16);
+}
+__device__ __forceinline__ void make_entry(Fp8x2& e, float a, float b) { e.v = float2_to_fp8x2(mid_of(a, b), slope_of(a, b)); }
 __device__ __forceinline__ void make_entry(float2& e, float a, float b) { e = make_float2(mid_of(a, b), slope_of(a, b)); }
 __device__ __forceinline__ void make_entry(unsigned& e, float a, float b) { e = pack_h2(mid_of(a, b), slope_of(a, b)); }
 
-constexpr int kEntriesPerThread = 4;
 constexpr int kThreads = 256;
 
-template <typename Out> struct alignas(16) Quad { Out e[kEntriesPerThread]; };
+template <typename Out, int EPT> struct alignas(EPT * sizeof(Out) >= 16 ? 16 : 8) Quad { Out e[EPT]; };
 
-// In = float2 (IQ) or float (RF); Out = entry type: float4 / uint2 (IQ fp32 / fp16),
-// float2 / unsigned (RF fp32 / fp16)
-template <typename In, typename Out>
+// In = float2 (IQ) or float (RF); Out = entry type: float4 / uint2 / Fp8x4 (IQ fp32 / fp16 / fp8),
+// float2 / unsigned / Fp8x2 (RF); kEntriesPerThread entries (>= 16 bytes) per thread
+template <typename In, typename Out, int kEntriesPerThread>
 __global__ void __launch_bounds__(kThreads)
 convert_kernel(const In* __restrict__ raw, Out* __restrict__ conv, int M, int Q, int K, int Kp,
                float scale) {
@@ -78,7 +81,7 @@ convert_kernel(const In* __restrict__ raw, Out* __restrict__ conv, int M, int Q,
       const int k = k0 + j;
       if (k >= 0 && k < K) y[j] = scaled(ldg_stream(src + k), scale); else zero(y[j]);
     }
-    Quad<Out> out;
+    Quad<Out, kEntriesPerThread> out;
     In z;
     zero(z);
 #pragma unroll
@@ -87,7 +90,7 @@ convert_kernel(const In* __restrict__ raw, Out* __restrict__ conv, int M, int Q,
       const bool ok = (k >= 0) && (k <= K - 2);              // both samples of the interval exist
       make_entry(out.e[j], ok ? y[j] : z, ok ? y[j + 1] : z);
     }
-    *reinterpret_cast<Quad<Out>*>(conv + row * Kp + (long long)ch * kEntriesPerThread) = out;
+    *reinterpret_cast<Quad<Out, kEntriesPerThread>*>(conv + row * Kp + (long long)ch * kEntriesPerThread) = out;
   }
 }
 
@@ -95,18 +98,21 @@ convert_kernel(const In* __restrict__ raw, Out* __restrict__ conv, int M, int Q,
 
 cudaError_t launch_convert(const Params& P, const void* d_raw, void* d_conv, float scale,
                            cudaStream_t s) {
-  const long long total = (long long)P.M * P.Q * (P.Kp / kEntriesPerThread);
+  const int ept = (!P.iq && P.fp8) ? 8 : 4;                  // RF fp8 entries are 2 bytes: 8 of them make 16
+  const long long total = (long long)P.M * P.Q * (P.Kp / ept);
   long long blocks = (total + kThreads - 1) / kThreads;
   const long long cap = 148LL * 8 * 16;                     // grid-stride beyond 16 waves
   if (blocks > cap) blocks = cap;
   if (blocks < 1) blocks = 1;
   dim3 grid((unsigned)blocks), block(kThreads);
   if (P.iq) {
-    if (P.fp16) convert_kernel<float2, uint2><<<grid, block, 0, s>>>((const float2*)d_raw, (uint2*)d_conv, P.M, P.Q, P.K, P.Kp, scale);
-    else        convert_kernel<float2, float4><<<grid, block, 0, s>>>((const float2*)d_raw, (float4*)d_conv, P.M, P.Q, P.K, P.Kp, scale);
+    if (P.fp8)       convert_kernel<float2, Fp8x4, 4><<<grid, block, 0, s>>>((const float2*)d_raw, (Fp8x4*)d_conv, P.M, P.Q, P.K, P.Kp, scale);
+    else if (P.fp16) convert_kernel<float2, uint2, 4><<<grid, block, 0, s>>>((const float2*)d_raw, (uint2*)d_conv, P.M, P.Q, P.K, P.Kp, scale);
+    else             convert_kernel<float2, float4, 4><<<grid, block, 0, s>>>((const float2*)d_raw, (float4*)d_conv, P.M, P.Q, P.K, P.Kp, scale);
   } else {
-    if (P.fp16) convert_kernel<float, unsigned><<<grid, block, 0, s>>>((const float*)d_raw, (unsigned*)d_conv, P.M, P.Q, P.K, P.Kp, scale);
-    else        convert_kernel<float, float2><<<grid, block, 0, s>>>((const float*)d_raw, (float2*)d_conv, P.M, P.Q, P.K, P.Kp, scale);
+    if (P.fp8)       convert_kernel<float, Fp8x2, 8><<<grid, block, 0, s>>>((const float*)d_raw, (Fp8x2*)d_conv, P.M, P.Q, P.K, P.Kp, scale);
+    else if (P.fp16) convert_kernel<float, unsigned, 4><<<grid, block, 0, s>>>((const float*)d_raw, (unsigned*)d_conv, P.M, P.Q, P.K, P.Kp, scale);
+    else             convert_kernel<float, float2, 4><<<grid, block, 0, s>>>((const float*)d_raw, (float2*)d_conv, P.M, P.Q, P.K, P.Kp, scale);
   }
   count_launch();
   return cudaGetLastError();

@@ -49,6 +49,20 @@ template <> struct Sample<unsigned> {     // RF fp16: half2 (mid, slope)
   }
 };
 
+template <> struct Sample<Fp8x4> {        // IQ fp8: 4 x e4m3 (mid.re, mid.im, slope.re, slope.im)
+  static __device__ __forceinline__ EntryF load(const Fp8x4* p) {
+    const unsigned u = __ldg(reinterpret_cast<const unsigned*>(p));
+    const float2 m = fp8x2_to_float2((unsigned short)(u & 0xffffu)), s = fp8x2_to_float2((unsigned short)(u >> 16));
+    return {m.x, m.y, s.x, s.y};
+  }
+};
+template <> struct Sample<Fp8x2> {        // RF fp8: 2 x e4m3 (mid, slope)
+  static __device__ __forceinline__ EntryF load(const Fp8x2* p) {
+    const float2 v = fp8x2_to_float2(__ldg(reinterpret_cast<const unsigned short*>(p)));
+    return {v.x, 0.f, v.y, 0.f};
+  }
+};
+
 template <bool IQ, typename T>
 __global__ void __launch_bounds__(kThreads)
 general_kernel(const Params P, const T* __restrict__ conv, void* __restrict__ out_v) {
@@ -222,11 +236,13 @@ cudaError_t launch_general(const Params& P, const void* d_conv, void* d_out, cud
   const long long N = (long long)P.nx * P.ny * P.nz;
   const unsigned blocks = (unsigned)((N + kThreads - 1) / kThreads);
   if (P.iq) {
-    if (P.fp16) general_kernel<true, uint2><<<blocks, kThreads, 0, s>>>(P, (const uint2*)d_conv, d_out);
-    else        general_kernel<true, float4><<<blocks, kThreads, 0, s>>>(P, (const float4*)d_conv, d_out);
+    if (P.fp8)       general_kernel<true, Fp8x4><<<blocks, kThreads, 0, s>>>(P, (const Fp8x4*)d_conv, d_out);
+    else if (P.fp16) general_kernel<true, uint2><<<blocks, kThreads, 0, s>>>(P, (const uint2*)d_conv, d_out);
+    else             general_kernel<true, float4><<<blocks, kThreads, 0, s>>>(P, (const float4*)d_conv, d_out);
   } else {
-    if (P.fp16) general_kernel<false, unsigned><<<blocks, kThreads, 0, s>>>(P, (const unsigned*)d_conv, d_out);
-    else        general_kernel<false, float2><<<blocks, kThreads, 0, s>>>(P, (const float2*)d_conv, d_out);
+    if (P.fp8)       general_kernel<false, Fp8x2><<<blocks, kThreads, 0, s>>>(P, (const Fp8x2*)d_conv, d_out);
+    else if (P.fp16) general_kernel<false, unsigned><<<blocks, kThreads, 0, s>>>(P, (const unsigned*)d_conv, d_out);
+    else             general_kernel<false, float2><<<blocks, kThreads, 0, s>>>(P, (const float2*)d_conv, d_out);
   }
   count_launch();
   return cudaGetLastError();

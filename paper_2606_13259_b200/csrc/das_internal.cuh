@@ -3,6 +3,7 @@
 #pragma once
 
 #include <cuda_fp16.h>
+#include <cuda_fp8.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -26,8 +27,21 @@ namespace das {
 //   IQ fp32: float4 (mid.re, mid.im, slope.re, slope.im)   16 B
 //   IQ fp16: 2 x __half2 (mid.re, mid.im | slope.re, slope.im) 8 B
 //   RF fp32: float2 (mid, slope) 8 B            RF fp16: __half2 (mid, slope) 4 B
+//   IQ fp8 : 4 x e4m3 (mid.re, mid.im, slope.re, slope.im) 4 B      RF fp8: 2 x e4m3 (mid, slope) 2 B
 // Element-major so that the Q rows one receiver contributes to a voxel tile sit side by side;
 // every row starts 16-byte aligned (Kp is a multiple of 8) for TMA bulk copies.
+struct Fp8x4 { unsigned v; };            // IQ fp8 entry
+struct Fp8x2 { unsigned short v; };      // RF fp8 entry
+// e4m3 pair -> two floats (hardware conversion through half precision, exact)
+__device__ __forceinline__ float2 fp8x2_to_float2(unsigned short v) {
+  const __half2_raw h = __nv_cvt_fp8x2_to_halfraw2((__nv_fp8x2_storage_t)v, __NV_E4M3);
+  return __half22float2(*reinterpret_cast<const __half2*>(&h));
+}
+__device__ __forceinline__ unsigned short float2_to_fp8x2(float lo, float hi) {
+  return (unsigned short)__nv_cvt_float2_to_fp8x2(make_float2(lo, hi), __NV_SATFINITE, __NV_E4M3);
+}
+// storage code of a plan: 0 fp32, 1 fp16, 2 fp8
+__host__ __device__ inline int storage_code(int fp16, int fp8) { return fp8 ? 2 : (fp16 ? 1 : 0); }
 constexpr int kPadLeft = 64;
 constexpr int kPadRight = 64;
 __host__ __device__ inline int padded_samples(int K) { return kPadLeft + ((K + 7) / 8) * 8 + kPadRight; }
@@ -44,6 +58,7 @@ struct Params {
   int nx, ny, nz;
   int iq;               // 1 = IQ (complex), 0 = RF
   int fp16;             // 1 = fp16 storage
+  int fp8;              // 1 = fp8 (e4m3) storage
   int apod;             // 1 = f-number boxcar active
   int has_dir;          // 1 = per-element normals given
   const float* xs;      // device copies of the axis vectors

@@ -55,13 +55,16 @@ constexpr unsigned kMagicBits = 0x4B400000u;
 constexpr float kBand = 4e-6f;                  // relative guard band of the FP32 aperture test
 static_assert(kConsumerWarps % 4 == 0 && kHelperWarps == 4 && kConvWarps + 1 <= kHelperWarps, "warpgroup roles");
 
-enum Mode { kIQ32 = 0, kIQ16 = 1, kRF32 = 2, kRF16 = 3 };
+enum Mode { kIQ32 = 0, kIQ16 = 1, kRF32 = 2, kRF16 = 3, kIQ8 = 4, kRF8 = 5 };
 template <int MODE> struct ModeTraits;   // eb: bytes of a stored (mid, slope) entry; tb: of a table entry
 template <> struct ModeTraits<kIQ32> { static constexpr bool iq = true;  static constexpr int eb = 16, tb = 16; };
 template <> struct ModeTraits<kIQ16> { static constexpr bool iq = true;  static constexpr int eb = 8,  tb = 16; };
 template <> struct ModeTraits<kRF32> { static constexpr bool iq = false; static constexpr int eb = 8,  tb = 8; };
 template <> struct ModeTraits<kRF16> { static constexpr bool iq = false; static constexpr int eb = 4,  tb = 8; };
-__host__ __device__ inline int entry_bytes(int iq, int fp16) { return (iq ? 2 : 1) * 2 * (fp16 ? 2 : 4); }
+template <> struct ModeTraits<kIQ8>  { static constexpr bool iq = true;  static constexpr int eb = 4,  tb = 16; };
+template <> struct ModeTraits<kRF8>  { static constexpr bool iq = false; static constexpr int eb = 2,  tb = 8; };
+// bytes of a stored (mid, slope) entry; st = storage code (0 fp32, 1 fp16, 2 fp8)
+__host__ __device__ inline int entry_bytes(int iq, int st) { return (iq ? 2 : 1) * 2 * (st == 0 ? 4 : (st == 1 ? 2 : 1)); }
 
 struct TileDesc {       // one voxel tile
   int ix0, iy0, iz0;    // origin (voxel indices)
@@ -127,6 +130,11 @@ __device__ __forceinline__ uint2 lds64u(unsigned addr) {
   asm volatile("ld.shared.v2.b32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
   return v;
 }
+__device__ __forceinline__ unsigned short lds16u(unsigned addr) {
+  unsigned short v;
+  asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr));
+  return v;
+}
 __device__ __forceinline__ unsigned lds32u(unsigned addr) {
   unsigned v;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v) : "r"(addr));
@@ -160,8 +168,8 @@ struct alignas(128) TiledSmem {
 };
 
 // upper bound of sizeof(TiledSmem<QC, W, MODE>) for the plan's occupancy estimate
-__host__ __device__ inline size_t tiled_smem_bytes(int QC, int W, int iq, int fp16) {
-  const size_t tb = iq ? 16 : 8, eb = (size_t)entry_bytes(iq, fp16);
+__host__ __device__ inline size_t tiled_smem_bytes(int QC, int W, int iq, int st) {
+  const size_t tb = iq ? 16 : 8, eb = (size_t)entry_bytes(iq, st);
   return (size_t)QC * W * (kTabStages * tb + kRawStages * eb) + (size_t)(iq ? QC : 1) * kConsumerThreads * 4 + 768;
 }
 
@@ -368,6 +376,13 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
               } else if constexpr (MODE == kIQ32) {
                 const float4 r = lds128<0>(src + j * 32 * EB);
                 sts128(dst + j * 32 * TB, make_float4(fmaf(-kl, r.z, r.x), fmaf(-kl, r.w, r.y), r.z, r.w));
+              } else if constexpr (MODE == kIQ8) {
+                const unsigned r = lds32u(src + j * 32 * EB);
+                const float2 mid = fp8x2_to_float2((unsigned short)(r & 0xffffu)), sl = fp8x2_to_float2((unsigned short)(r >> 16));
+                sts128(dst + j * 32 * TB, make_float4(fmaf(-kl, sl.x, mid.x), fmaf(-kl, sl.y, mid.y), sl.x, sl.y));
+              } else if constexpr (MODE == kRF8) {
+                const float2 ms = fp8x2_to_float2(lds16u(src + j * 32 * EB));
+                sts64(dst + j * 32 * TB, make_float2(fmaf(-kl, ms.y, ms.x), ms.y));
               } else if constexpr (MODE == kRF16) {
                 const unsigned r = lds32u(src + j * 32 * EB);
                 const float2 ms = __half22float2(*reinterpret_cast<const __half2*>(&r));
@@ -538,6 +553,8 @@ cudaError_t launch_tiled_iq32(int QC, int W, const TiledDev&, const Params&, con
 cudaError_t launch_tiled_iq16(int QC, int W, const TiledDev&, const Params&, const void*, void*, int grid, cudaStream_t);
 cudaError_t launch_tiled_rf32(int QC, int W, const TiledDev&, const Params&, const void*, void*, int grid, cudaStream_t);
 cudaError_t launch_tiled_rf16(int QC, int W, const TiledDev&, const Params&, const void*, void*, int grid, cudaStream_t);
+cudaError_t launch_tiled_iq8(int QC, int W, const TiledDev&, const Params&, const void*, void*, int grid, cudaStream_t);
+cudaError_t launch_tiled_rf8(int QC, int W, const TiledDev&, const Params&, const void*, void*, int grid, cudaStream_t);
 
 constexpr int kWindows[] = {16, 20, 24, 32, 48, 64};
 

@@ -58,7 +58,8 @@ TiledPlan* tiled_plan_create(const Params& P, const das_plan_desc_t& d, int devi
   const bool apod = fnum > 0.0;
   const double kappa = fs / c;
   const int Q = d.n_tx, M = d.n_elem;
-  const int align = 16 / entry_bytes(P.iq, P.fp16);     // window origins in units the TMA copy accepts
+  const int st = storage_code(P.fp16, P.fp8);
+  const int align = 16 / entry_bytes(P.iq, st);         // window origins in units the TMA copy accepts
   const int TXv = kWX * kLaneX, TYv = kWY * kLaneY, TZv = kWZ;
   const int ntx = (d.nx + TXv - 1) / TXv, nty = (d.ny + TYv - 1) / TYv, ntz = (d.nz + TZv - 1) / TZv;
   const long long n_tiles_ll = (long long)ntx * nty * ntz;
@@ -167,7 +168,8 @@ TiledPlan* tiled_plan_create(const Params& P, const das_plan_desc_t& d, int devi
 
   // entry index = round(Tf + e') with Tf + e' in [1/2, span_t + span_e - 1/2]: it must stay <= W - 1
   int W = 0;
-  for (int cand : kWindows) if (w_needed + 0.02 <= (double)cand) { W = cand; break; }
+  for (int cand : kWindows)                                // a staged row (W entries) must be a whole number of 16-byte units
+    if (w_needed + 0.02 <= (double)cand && (cand * entry_bytes(P.iq, st)) % 16 == 0) { W = cand; break; }
   if (!W) { snprintf(why, why_len, "sample window per tile (%.1f samples) exceeds the largest staged window (%d)", w_needed, kWindows[sizeof(kWindows) / sizeof(int) - 1]); return nullptr; }
 
   // order tiles by decreasing work (static round-robin schedule over persistent CTAs)
@@ -186,7 +188,7 @@ TiledPlan* tiled_plan_create(const Params& P, const das_plan_desc_t& d, int devi
   cudaDeviceProp prop;
   cudaError_t e = cudaGetDeviceProperties(&prop, device);
   if (e != cudaSuccess) { *cuda_err = e; delete tp; return nullptr; }
-  const size_t smem = tiled_smem_bytes(QC, W, P.iq, P.fp16);
+  const size_t smem = tiled_smem_bytes(QC, W, P.iq, st);
   const int ctas_per_sm = (smem + 1024) * 2 <= (size_t)prop.sharedMemPerMultiprocessor ? 2 : 1;
   tp->grid = std::max(1, std::min(n_tiles, prop.multiProcessorCount * ctas_per_sm));
   TiledDev& dv = tp->dev;
@@ -208,6 +210,8 @@ cudaError_t launch_tiled(const TiledPlan* tp, const Params& P, const void* d_con
                          cudaStream_t s, int* n_launches) {
   *n_launches = 1;
   count_launch();
+  if (P.fp8) return P.iq ? launch_tiled_iq8(tp->QC, tp->W, tp->dev, P, d_conv, d_out, tp->grid, s)
+                         : launch_tiled_rf8(tp->QC, tp->W, tp->dev, P, d_conv, d_out, tp->grid, s);
   if (P.iq) return P.fp16 ? launch_tiled_iq16(tp->QC, tp->W, tp->dev, P, d_conv, d_out, tp->grid, s)
                           : launch_tiled_iq32(tp->QC, tp->W, tp->dev, P, d_conv, d_out, tp->grid, s);
   return P.fp16 ? launch_tiled_rf16(tp->QC, tp->W, tp->dev, P, d_conv, d_out, tp->grid, s)
