@@ -47,7 +47,8 @@ if ROOT not in sys.path:
 
 import numpy as np
 
-METRIC = "volumes/s at 128^3 vox, 1024 el, 16 tx"
+METRIC = "volumes/s at 128^3 vox, 1024 el, 16 tx"       # BASELINE.json; `value` is at config.frames_per_call frames
+                                                       # per das_execute, `value_one_frame_per_call` at one
 UNIT = "volumes/s"
 
 # Definition flops per unit of algorithmic work:
@@ -59,12 +60,29 @@ FLOPS_PER_PAIR = 28.0
 FP32_LANES_PER_SM = 128          # B200_PROFILING.md / B300_MICROARCH.md: 4 SMSP x 32 lanes
 N_SM = 148
 
-# dram__bytes_read.sum + dram__bytes_write.sum of the tiled kernel, per launch, from the
-# `ncu --set full` capture summarised in profiles/ (bytes); keyed by (config, storage).
-NCU_TRAFFIC_BYTES = {
-    (3, "fp16", 1): 57.05e6,     # profiles/r1_tiled_v3_iq16_full.md
-    (3, "fp16", 64): 175.3e9,    # profiles/r1_tc_b64_full.md
-}
+PROFILES = os.path.join(ROOT, "profiles")
+
+
+def load_profile(name):
+    """ncu counters of one kernel from the committed summary profiles/<name>.json (written from an
+    `ncu --set full` report by `python -m paper_2606_13259_b200.ncu_summary`), or None.  Nothing profiler-
+    derived is typed into this file: what the bench prints under "traffic" / "ncu" is read from there and
+    labelled with the file it came from."""
+    try:
+        with open(os.path.join(PROFILES, name + ".json")) as f:
+            d = json.load(f)
+        d["source"] = f"profiles/{name}.json"
+        return d
+    except Exception:
+        return None
+
+
+def bound_from_profile(prof, default):
+    """the binding roofline is the largest of the utilisation counters of the capture."""
+    if not prof or "utilisation_pct" not in prof:
+        return default, None
+    name, pct = max(prof["utilisation_pct"].items(), key=lambda kv: kv[1])
+    return name, pct
 
 
 def parse_args():
@@ -229,6 +247,24 @@ def run_reference(args):
 BAD_REASONS = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"}
 
 
+def rank_barrier(dist, sync=None):
+    """Barrier over the ranks (torch.distributed, if initialised) followed by a device synchronise."""
+    if dist is not None:
+        dist.barrier()
+    if sync is not None:
+        sync()
+
+
+def rank_max(dist, x, device=None):
+    """Max over the ranks of one float (the device time of the timed region); the plain value for one rank."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def make_frames(w, n_frames):
     """Frame 0 is the config's seeded channel data; frames f > 0 add an independent seeded
     noise realisation (sigma 0.01) so that every timed step reads different bytes.  The rotation
@@ -264,12 +300,16 @@ def fp32_peak_tflops(sampler_max_mhz):
 
 
 def tensor_peak_tflops():
-    """Dense FP16 tensor peak: the driver-measured bf16 cuBLAS burst figure of MEASURED_PEAKS.json
-    (FP16 and BF16 run at the same rate; the batch kernel is timed alone, launch by launch),
-    else the B200_PROFILING.md nominal 2250 TFLOP/s."""
+    """Dense FP16 tensor peak from MEASURED_PEAKS.json (driver-written, bf16 cuBLAS; FP16 and BF16 run at the
+    same rate).  The batch kernel is timed inside a long, power-capped step loop, so the denominator is the
+    SUSTAINED figure (B200_PROFILING.md); the burst figure is returned beside it.  Fallback: the guide's
+    nominal 2250 TFLOP/s."""
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-            return float(json.load(f)["bf16_tflops"]), "MEASURED_PEAKS.json bf16_tflops (burst), same rate for fp16"
+            d = json.load(f)
+        sus, burst = float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), float(d["bf16_tflops"])
+        return sus, (f"MEASURED_PEAKS.json bf16_tflops_sustained = {sus:.0f} TFLOP/s (kernel timed inside a long step; "
+                     f"burst {burst:.0f}), same rate for fp16")
     except Exception:
         return 2250.0, "B200_PROFILING.md nominal dense bf16/fp16 (fallback)"
 
@@ -314,16 +354,10 @@ def run_cuda(args):
     das.load()                                   # raises if libdas_b200.so is missing
 
     def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
+        rank_barrier(dist, torch.cuda.synchronize)
 
     def max_over_ranks(x):
-        if dist is None:
-            return float(x)
-        t = torch.tensor([float(x)], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return rank_max(dist, x, dev)
 
     w = wl.config(args.config)
     batchable = w.data_kind == 0 and args.storage == "fp16"
@@ -378,16 +412,26 @@ def run_cuda(args):
         steps = s1_steps
         algo_used = algo1
     else:
-        # ---- B frames per call: the frame-batch tensor-core kernel.  The batch holds the rotated
-        # seeded frames under exact power-of-two scales (64 distinct frames, 8.6 GB of raw input per
-        # step at the headline: no step finds its input in the 126 MB L2).
+        # ---- B frames per call: the frame-batch tensor-core kernel.  At the headline the batch is
+        # BASELINE.json configs[4] (the streaming ensemble): `--frames` (4) seeded config-5 frames from
+        # workloads.streaming_frames (drifting scatterers over +20 dB clutter), each used B / 4 times under
+        # an exact power-of-two scale (2^0 .. 2^-3): B / 4 x 4 = 16 distinct frames among the 64 slots, the
+        # same input pattern tests/test_gpu_tc.py checks against the oracle.  8.6 GB of raw input per
+        # step: no step finds its input in the 126 MB L2.
         plan = das.Plan.from_workload(w, storage=storage, algo=das.ALGO_AUTO, device=local_rank, n_frames=B)
         if plan.algo != das.ALGO_TC:
             raise SystemExit("bench.py: the tensor-core batch kernel does not apply to this configuration")
         algo_used = "tensor-core batch"
+        if args.config == 3:
+            base = [torch.from_numpy(np.ascontiguousarray(f.y)).to(dev) for f in wl.streaming_frames(max(1, args.frames))]
+            batch_data = f"configs[4]: {len(base)} seeded streaming frames x {B // len(base)} power-of-two scales"
+        else:
+            base = raw1
+            batch_data = f"{len(base)} seeded frames (config data + noise realisations) x power-of-two scales"
         rawB = torch.empty((B,) + tuple(w.y.shape), dtype=raw1[0].dtype, device=dev)
         for b in range(B):
-            rawB[b] = raw1[b % len(raw1)] * (2.0 ** (-((b // len(raw1)) % 4)))
+            rawB[b] = base[b % len(base)] * (2.0 ** (-((b // len(base)) % 4)))
+        del base
         raws = [rawB]
         out = torch.empty((B,) + tuple(w.grid_shape), dtype=out_dt, device=dev)
         steps = args.steps
@@ -399,18 +443,35 @@ def run_cuda(args):
     else:
         h_raw = [torch.empty(tuple(rawB.shape), dtype=rawB.dtype, pin_memory=True)]
         h_raw[0].copy_(rawB)
-    h_out = torch.empty(tuple(out.shape), dtype=out.dtype).pin_memory()
+    # two output buffers: the pipelined API keeps two calls in flight (das.h das_beamform_host_begin / _wait)
+    h_outs = [torch.empty(tuple(out.shape), dtype=out.dtype).pin_memory() for _ in range(2)]
+    h_out = h_outs[0]
     plan.beamform_host(h_raw[0].data_ptr(), h_out.data_ptr(), sp)          # allocates the staging
-    e_steps = max(1, args.e2e_steps if B == 1 else min(args.e2e_steps, 3))
+    e_steps = max(2, args.e2e_steps if B == 1 else min(args.e2e_steps, 4))
     e_beg, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
+    t_wall = time.perf_counter()
     e_beg.record(stream)
-    for i in range(e_steps):
-        plan.beamform_host(h_raw[i % len(h_raw)].data_ptr(), h_out.data_ptr(), sp)
-    e_end.record(stream)
+    plan.beamform_host_begin(h_raw[0].data_ptr(), h_outs[0].data_ptr(), sp)
+    for i in range(1, e_steps):
+        plan.beamform_host_begin(h_raw[i % len(h_raw)].data_ptr(), h_outs[i % 2].data_ptr(), sp)
+        plan.beamform_host_wait()                                         # result i - 1 is in host memory
+    plan.beamform_host_wait()
+    e2e_wall_ms = (time.perf_counter() - t_wall) * 1e3                    # the last D2H runs on the plan's copy stream:
+    e_end.record(stream)                                                  # the host clock around begin .. wait covers it
     stream.synchronize()
     barrier()
-    e2e_ms = max_over_ranks(e_beg.elapsed_time(e_end))
+    e2e_ms = max_over_ranks(max(e_beg.elapsed_time(e_end), e2e_wall_ms))
+    h_out = h_outs[(e_steps - 1) % 2]
+    # host -> device copy of one step's input alone (configs[4]: "host-to-device copies timed separately")
+    h_beg, h_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stage = raws[0]
+    h_beg.record(stream)
+    with torch.cuda.stream(stream):
+        stage.copy_(h_raw[0], non_blocking=True)
+    h_end.record(stream)
+    stream.synchronize()
+    h2d_ms = h_beg.elapsed_time(h_end)
     checksum = float(h_out.abs().max())                                   # the D2H result is read
 
     if rank != 0:
@@ -419,12 +480,16 @@ def run_cuda(args):
         return 0
 
     value = world * B * steps / (total_ms * 1e-3)
+    # ncu counters of the two kernels: read from the committed summaries, never typed in here
+    prof_tc = load_profile("r2_tc_b64_full")
+    prof_tiled = load_profile("r2_tiled_iq16_full") if (args.config == 3 and args.storage == "fp16") else None
     if B == 1:
         flops = flops1
         peak, peak_how = fp32_peak_tflops(clocks.get("sm_max_mhz"))
-        bound, peak_how = "alu", peak_how + ", derived (no measured FP32 peak)"
+        peak_how += ", derived (no measured FP32 peak)"
+        bound = "alu"
         flops_model = (f"{FLOPS_PER_TERM[w.data_kind]:.0f} x entered terms + {FLOPS_PER_PAIR:.0f} x active (m,n) pairs (DESIGN.md)")
-        extra = {}
+        prof = prof_tiled if algo_used == "tiled" else None
     else:
         # per frame every entered term is interpolated, rotated and accumulated (17 definition flops);
         # the geometry of an active (m, n) pair is worked out once per batch
@@ -432,11 +497,17 @@ def run_cuda(args):
         peak, peak_how = tensor_peak_tflops()
         bound = "tensor"
         flops_model = (f"{FLOPS_PER_TERM[w.data_kind]:.0f} x entered terms x {B} frames + {FLOPS_PER_PAIR:.0f} x active (m,n) pairs "
-                       f"(DESIGN.md); the MMAs the kernel issues carry 4x to 5x as many (2 of 8 samples of a K = 16 pass are non-zero)")
-        extra = {"ncu": {"tensor_pipe_active": 0.44, "issue_slots_active": 0.64, "alu_pipe_active": 0.62,
-                         "source": "profiles/r1_tc_b64_full.md"}}
+                       f"(DESIGN.md); a K = 16 MMA pass carries 8 samples per voxel row of which 2 are non-zero, so the MMAs "
+                       f"the kernel issues carry about 4.7x as many")
+        prof = prof_tc if (args.config == 3 and B == 64) else None
+    extra = {}
+    traffic = None
+    if prof:
+        traffic = prof.get("dram_bytes")
+        extra = {"ncu": {k: prof[k] for k in ("utilisation_pct", "dram_bytes_read", "dram_bytes_write", "l2_hit_rate_pct",
+                                                "warp_instructions", "gpu_time_ms", "kernel", "source", "command") if k in prof}}
+        extra["ncu"]["binding_counter"] = dict(zip(("name", "pct"), bound_from_profile(prof, bound)))
     achieved = flops / (exec_ms * 1e-3) / 1e12
-    traffic = NCU_TRAFFIC_BYTES.get((args.config, args.storage, B)) if algo_used != "general" else None
     raw_bytes = sum(r.nbytes for r in raws)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
@@ -447,7 +518,8 @@ def run_cuda(args):
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"{raw_bytes / 1e6:.0f} MB of distinct raw input per rotation + {convbytes / 1e6:.0f} MB converted "
                          f"buffer rewritten every step > 126 MB L2",
-                   "step": f"das_convert + das_execute on device-resident input, {B} frame(s) per call"},
+                   "step": f"das_convert + das_execute on device-resident input, {B} frame(s) per call",
+                   "batch_data": batch_data if B > 1 else None},
         "accumulations_per_s": {"nominal": w.nominal_accumulations * value, "entered": n_terms * value,
                                 "nominal_per_volume": w.nominal_accumulations, "entered_per_volume": n_terms,
                                 "active_pairs_per_volume": n_pairs},
@@ -459,14 +531,25 @@ def run_cuda(args):
                           "flops_per_launch": flops, "flops_model": flops_model, "peak_how": peak_how}, **extra),
         "e2e": {"value": world * B * e_steps / (e2e_ms * 1e-3), "unit": UNIT,
                 "h2d_bytes_per_step": int(plan.raw_bytes), "d2h_bytes_per_step": int(plan.output_bytes),
-                "ms_per_step": e2e_ms / e_steps, "steps": e_steps, "api": "das_beamform_host, pinned host buffers",
+                "ms_per_step": e2e_ms / e_steps, "steps": e_steps,
+                "api": "das_beamform_host_begin / _wait, two calls in flight, pinned host buffers",
+                "h2d_alone_ms": h2d_ms, "h2d_alone_gbs": plan.raw_bytes / (h2d_ms * 1e-3) / 1e9,
                 "checksum_max_abs": checksum},
         "gpu_launches": int(launches),
         "clocks": clocks,
         "single_frame": dict(single, roofline={"bound": "alu", "achieved": flops1 / (exec1 * 1e-3) / 1e12,
                                                "peak": fp32_peak_tflops(clocks.get("sm_max_mhz"))[0], "unit": "TFLOP/s"}),
     }
-    line["single_frame"]["roofline"]["frac"] = line["single_frame"]["roofline"]["achieved"] / line["single_frame"]["roofline"]["peak"]
+    sf = line["single_frame"]["roofline"]
+    sf["frac"] = sf["achieved"] / sf["peak"]
+    if prof_tiled and algo1 == "tiled":
+        # the binding roofline of the one-frame kernel is the largest utilisation counter of its capture
+        name, pct = bound_from_profile(prof_tiled, "alu")
+        sf["binding_counter"] = {"name": name, "pct": pct, "source": prof_tiled["source"]}
+        sf["traffic"] = prof_tiled.get("dram_bytes")
+    # both readings of the metric at top level: B frames per call (value) and one frame per call
+    line["value_frames_per_call"] = B
+    line["value_one_frame_per_call"] = line["single_frame"]["value"]
     if world == 1 and args.cpu_seconds > 0:
         line["cpu_baseline"] = cpu_baseline(w, args.cpu_seconds)
     else:

@@ -155,6 +155,19 @@ das_status_t das_execute(const das_plan_t* plan, const void* d_conv, void* d_out
  * copy bandwidth h_raw / h_out should be page-locked. */
 das_status_t das_beamform_host(das_plan_t* plan, const void* h_raw, void* h_out, void* stream);
 
+/* The same as a two-deep pipeline for streaming callers (BASELINE.json configs[4]: frames arrive from the
+ * host one batch after another).  das_beamform_host_begin enqueues the host-to-device copy of h_raw on a
+ * copy stream of the plan, das_convert + das_execute on `stream`, and the device-to-host copy into h_out on
+ * a second copy stream, chained by events, and returns without waiting; das_beamform_host_wait blocks until
+ * the OLDEST outstanding call has delivered its h_out.  At most two calls may be outstanding (the plan owns
+ * two raw / output staging buffers and one converted buffer); a third begin returns DAS_ERR_INVALID_ARG.
+ * With two calls in flight the copies of one batch run under the kernels of the other, so the sustained rate
+ * is that of the slower of the two (PCIe for the headline batch: 8.6 GB in, 1.1 GB out per 64 frames).
+ * h_raw must stay valid until the matching wait returns; both buffers should be page-locked.  Always pass the
+ * same `stream` for one plan.  das_beamform_host == begin + wait. */
+das_status_t das_beamform_host_begin(das_plan_t* plan, const void* h_raw, void* h_out, void* stream);
+das_status_t das_beamform_host_wait(das_plan_t* plan);
+
 /* Work accounting (used by the bench's roofline; not part of the hot path).  Runs a counting
  * kernel on the plan's device and SYNCHRONISES.  On success
  *   *n_pairs = number of (m, n) receiver/voxel pairs with non-zero receive weight w_rx

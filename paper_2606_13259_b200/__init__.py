@@ -33,6 +33,7 @@ INTERP_LINEAR, INTERP_CUBIC = 0, 1
 # every symbol include/das.h declares (checked against the header by tests/test_abi.py)
 EXPORTS = ("das_plan_create", "das_plan_destroy", "das_raw_bytes", "das_converted_bytes",
            "das_output_bytes", "das_plan_algo", "das_plan_frames", "das_convert", "das_execute", "das_beamform_host",
+           "das_beamform_host_begin", "das_beamform_host_wait",
            "das_plan_count_work", "das_status_string", "das_last_error", "das_launch_count")
 
 
@@ -102,6 +103,10 @@ def load(build_if_missing: bool = True):
     lib.das_execute.argtypes = [vp, vp, vp, vp]
     lib.das_beamform_host.restype = ctypes.c_int
     lib.das_beamform_host.argtypes = [vp, vp, vp, vp]
+    lib.das_beamform_host_begin.restype = ctypes.c_int
+    lib.das_beamform_host_begin.argtypes = [vp, vp, vp, vp]
+    lib.das_beamform_host_wait.restype = ctypes.c_int
+    lib.das_beamform_host_wait.argtypes = [vp]
     lib.das_plan_count_work.restype = ctypes.c_int
     lib.das_plan_count_work.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong), ctypes.POINTER(ctypes.c_ulonglong)]
     lib.das_status_string.restype = ctypes.c_char_p
@@ -237,6 +242,13 @@ class Plan:
     def beamform_host(self, h_raw: int, h_out: int, stream: int = 0):
         _check(self._lib.das_beamform_host(self._h, ctypes.c_void_p(h_raw), ctypes.c_void_p(h_out),
                                            ctypes.c_void_p(stream)))
+
+    def beamform_host_begin(self, h_raw: int, h_out: int, stream: int = 0):
+        _check(self._lib.das_beamform_host_begin(self._h, ctypes.c_void_p(h_raw), ctypes.c_void_p(h_out),
+                                                 ctypes.c_void_p(stream)))
+
+    def beamform_host_wait(self):
+        _check(self._lib.das_beamform_host_wait(self._h))
 
     def count_work(self):
         """(n_pairs, n_terms) of das_plan_count_work: active (m, n) pairs and entered (q, m, n) terms."""

@@ -60,10 +60,16 @@ struct das_plan {
   TcPlan* tc = nullptr;
   int frames = 1;                         // B
   size_t raw1 = 0, conv1 = 0, out1 = 0;   // per-frame sizes (frame-by-frame path)
-  // staging for das_beamform_host (lazy)
-  void* st_raw = nullptr;
+  // staging for das_beamform_host[_begin / _wait] (lazy): two raw / output slots, one converted buffer
+  struct HostSlot {
+    void* d_raw = nullptr;
+    void* d_out = nullptr;
+    cudaEvent_t ev_h2d = nullptr, ev_exec = nullptr, ev_d2h = nullptr;
+    bool used = false;           // ev_exec / ev_d2h have been recorded at least once
+  } slot[2];
   void* st_conv = nullptr;
-  void* st_out = nullptr;
+  cudaStream_t s_in = nullptr, s_out = nullptr;
+  unsigned long long begun = 0, waited = 0;
 };
 
 static void free_plan(das_plan* p) {
@@ -72,9 +78,16 @@ static void free_plan(das_plan* p) {
   if (p->tiled) tiled_plan_destroy(p->tiled);
   if (p->tc) tc_plan_destroy(p->tc);
   for (void* d : p->dev_allocs) cudaFree(d);
-  if (p->st_raw) cudaFree(p->st_raw);
+  for (auto& sl : p->slot) {
+    if (sl.d_raw) cudaFree(sl.d_raw);
+    if (sl.d_out) cudaFree(sl.d_out);
+    if (sl.ev_h2d) cudaEventDestroy(sl.ev_h2d);
+    if (sl.ev_exec) cudaEventDestroy(sl.ev_exec);
+    if (sl.ev_d2h) cudaEventDestroy(sl.ev_d2h);
+  }
   if (p->st_conv) cudaFree(p->st_conv);
-  if (p->st_out) cudaFree(p->st_out);
+  if (p->s_in) cudaStreamDestroy(p->s_in);
+  if (p->s_out) cudaStreamDestroy(p->s_out);
   delete p;
 }
 
@@ -362,33 +375,78 @@ das_status_t das_execute(const das_plan_t* p, const void* d_conv, void* d_out, v
   return DAS_OK;
 }
 
-das_status_t das_beamform_host(das_plan_t* p, const void* h_raw, void* h_out, void* stream) {
+static das_status_t host_staging(das_plan* p) {
+  if (p->st_conv) return DAS_OK;
+  cudaError_t e = cudaSuccess;
+  auto fail = [&](const char* what) {
+    cuda_fail(e, what);
+    for (auto& sl : p->slot) {
+      if (sl.d_raw) { cudaFree(sl.d_raw); sl.d_raw = nullptr; }
+      if (sl.d_out) { cudaFree(sl.d_out); sl.d_out = nullptr; }
+    }
+    if (p->st_conv) { cudaFree(p->st_conv); p->st_conv = nullptr; }
+    return e == cudaErrorMemoryAllocation ? DAS_ERR_ALLOC : DAS_ERR_CUDA;
+  };
+  for (auto& sl : p->slot) {
+    if ((e = cudaMalloc(&sl.d_raw, p->raw_bytes)) != cudaSuccess || (e = cudaMalloc(&sl.d_out, p->out_bytes)) != cudaSuccess)
+      return fail("allocating staging buffers");
+    if (!sl.ev_h2d && ((e = cudaEventCreateWithFlags(&sl.ev_h2d, cudaEventDisableTiming)) != cudaSuccess ||
+                       (e = cudaEventCreateWithFlags(&sl.ev_exec, cudaEventDisableTiming)) != cudaSuccess ||
+                       (e = cudaEventCreateWithFlags(&sl.ev_d2h, cudaEventDisableTiming)) != cudaSuccess))
+      return fail("creating events");
+  }
+  if (!p->s_in && ((e = cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking)) != cudaSuccess ||
+                   (e = cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking)) != cudaSuccess))
+    return fail("creating copy streams");
+  if ((e = cudaMalloc(&p->st_conv, p->conv_bytes)) != cudaSuccess) return fail("allocating staging buffers");
+  return DAS_OK;
+}
+
+das_status_t das_beamform_host_begin(das_plan_t* p, const void* h_raw, void* h_out, void* stream) {
   if (!p || !h_raw || !h_out) { set_err("das_beamform_host: NULL argument"); return DAS_ERR_INVALID_ARG; }
+  if (p->begun - p->waited >= 2) { set_err("das_beamform_host_begin: two calls are outstanding already"); return DAS_ERR_INVALID_ARG; }
   DeviceGuard g(p->device);
   if (!g.ok) return cuda_fail(g.err, "selecting the CUDA device");
-  cudaError_t e;
-  if (!p->st_raw) {
-    if ((e = cudaMalloc(&p->st_raw, p->raw_bytes)) != cudaSuccess ||
-        (e = cudaMalloc(&p->st_conv, p->conv_bytes)) != cudaSuccess ||
-        (e = cudaMalloc(&p->st_out, p->out_bytes)) != cudaSuccess) {
-      cuda_fail(e, "allocating staging buffers");
-      if (p->st_raw) { cudaFree(p->st_raw); p->st_raw = nullptr; }
-      if (p->st_conv) { cudaFree(p->st_conv); p->st_conv = nullptr; }
-      if (p->st_out) { cudaFree(p->st_out); p->st_out = nullptr; }
-      return DAS_ERR_ALLOC;
-    }
-  }
+  das_status_t st = host_staging(p);
+  if (st != DAS_OK) return st;
+  das_plan::HostSlot& sl = p->slot[p->begun & 1];
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  if ((e = cudaMemcpyAsync(p->st_raw, h_raw, p->raw_bytes, cudaMemcpyHostToDevice, s)) != cudaSuccess)
+  cudaError_t e;
+  // slot reuse: the previous user's kernels have read d_raw (ev_exec), its copy-out has read d_out (ev_d2h)
+  if (sl.used && (e = cudaStreamWaitEvent(p->s_in, sl.ev_exec, 0)) != cudaSuccess) return cuda_fail(e, "stream wait");
+  if ((e = cudaMemcpyAsync(sl.d_raw, h_raw, p->raw_bytes, cudaMemcpyHostToDevice, p->s_in)) != cudaSuccess)
     return cuda_fail(e, "host-to-device copy");
-  das_status_t st = das_convert(p, p->st_raw, p->st_conv, 1.0f, stream);
-  if (st != DAS_OK) return st;
-  st = das_execute(p, p->st_conv, p->st_out, stream);
-  if (st != DAS_OK) return st;
-  if ((e = cudaMemcpyAsync(h_out, p->st_out, p->out_bytes, cudaMemcpyDeviceToHost, s)) != cudaSuccess)
+  if ((e = cudaEventRecord(sl.ev_h2d, p->s_in)) != cudaSuccess || (e = cudaStreamWaitEvent(s, sl.ev_h2d, 0)) != cudaSuccess ||
+      (sl.used && (e = cudaStreamWaitEvent(s, sl.ev_d2h, 0)) != cudaSuccess))
+    return cuda_fail(e, "event chain");
+  if ((st = das_convert(p, sl.d_raw, p->st_conv, 1.0f, stream)) != DAS_OK) return st;
+  if ((st = das_execute(p, p->st_conv, sl.d_out, stream)) != DAS_OK) return st;
+  if ((e = cudaEventRecord(sl.ev_exec, s)) != cudaSuccess || (e = cudaStreamWaitEvent(p->s_out, sl.ev_exec, 0)) != cudaSuccess)
+    return cuda_fail(e, "event chain");
+  if ((e = cudaMemcpyAsync(h_out, sl.d_out, p->out_bytes, cudaMemcpyDeviceToHost, p->s_out)) != cudaSuccess)
     return cuda_fail(e, "device-to-host copy");
-  if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return cuda_fail(e, "stream synchronize");
+  if ((e = cudaEventRecord(sl.ev_d2h, p->s_out)) != cudaSuccess) return cuda_fail(e, "event record");
+  sl.used = true;
+  ++p->begun;
   return DAS_OK;
+}
+
+das_status_t das_beamform_host_wait(das_plan_t* p) {
+  if (!p) { set_err("das_beamform_host_wait: NULL plan"); return DAS_ERR_INVALID_ARG; }
+  if (p->begun == p->waited) { set_err("das_beamform_host_wait: nothing outstanding"); return DAS_ERR_INVALID_ARG; }
+  DeviceGuard g(p->device);
+  if (!g.ok) return cuda_fail(g.err, "selecting the CUDA device");
+  cudaError_t e = cudaEventSynchronize(p->slot[p->waited & 1].ev_d2h);
+  ++p->waited;
+  if (e != cudaSuccess) return cuda_fail(e, "waiting for the device-to-host copy");
+  return DAS_OK;
+}
+
+das_status_t das_beamform_host(das_plan_t* p, const void* h_raw, void* h_out, void* stream) {
+  if (p && p->begun != p->waited) { set_err("das_beamform_host: pipelined calls are outstanding; wait for them first"); return DAS_ERR_INVALID_ARG; }
+  das_status_t st = das_beamform_host_begin(p, h_raw, h_out, stream);
+  if (st != DAS_OK) return st;
+  return das_beamform_host_wait(p);
 }
 
 das_status_t das_plan_count_work(const das_plan_t* p, unsigned long long* n_pairs, unsigned long long* n_terms) {

@@ -28,17 +28,22 @@ def test_reference_arm_two_ranks_prints_one_line():
 
 
 def test_max_over_ranks_and_barrier_gloo(tmp_path):
-    """The reduction bench.py uses for its timing (all_reduce MAX after a barrier), on gloo."""
+    """bench.py's own timing helpers (rank_barrier, rank_max: a barrier, then all_reduce MAX of the device
+    time) on gloo, world_size 2: every rank must see the slower rank's time."""
     script = tmp_path / "w.py"
     script.write_text(
-        "import os, torch, torch.distributed as dist\n"
+        "import sys, torch.distributed as dist\n"
+        f"sys.path.insert(0, {ROOT!r})\n"
+        "import bench\n"
         "dist.init_process_group('gloo')\n"
         "rank = dist.get_rank()\n"
-        "dist.barrier()\n"
-        "t = torch.tensor([10.0 + 5.0 * rank], dtype=torch.float64)\n"
-        "dist.all_reduce(t, op=dist.ReduceOp.MAX)\n"
-        "assert float(t.item()) == 15.0\n"
-        "if rank == 0: print('MAX', float(t.item()))\n"
+        "synced = []\n"
+        "bench.rank_barrier(dist, lambda: synced.append(1))\n"
+        "assert synced == [1]\n"
+        "t = bench.rank_max(dist, 10.0 + 5.0 * rank)\n"
+        "assert t == 15.0, t\n"
+        "assert bench.rank_max(None, 7.5) == 7.5\n"
+        "if rank == 0: print('MAX', t)\n"
         "dist.destroy_process_group()\n")
     r = _torchrun([str(script)], 29732)
     assert r.returncode == 0, r.stderr[-2000:]

@@ -225,3 +225,35 @@ def test_tc_beamform_host_batch(das_lib):
     np.testing.assert_array_equal(h_out.numpy(), dev.cpu().numpy())
     check_frames(h_out.numpy(), w, yb, frames=[0, 7], label="beamform_host B=8")
     plan.destroy()
+
+
+def test_tc_beamform_host_pipelined(das_lib):
+    """das_beamform_host_begin / _wait (das.h): two calls in flight, three batches through two host output
+    buffers; every result equals the device-resident path bit for bit, the protocol errors are reported."""
+    das, torch = das_lib, _torch()
+    w = _cfg(1, (17, 9, 6))
+    batches = [make_batch(w.y, 8, 120 + i) for i in range(3)]
+    plan = das.Plan.from_workload(w, storage=das.STORE_FP16, algo=das.ALGO_TC, n_frames=8)
+    want = []
+    for yb in batches:
+        dev, _ = das.beamform_torch(plan, torch.from_numpy(yb).cuda())
+        torch.cuda.synchronize()
+        want.append(dev.cpu().numpy())
+    h_raw = [torch.from_numpy(yb).pin_memory() for yb in batches]
+    h_out = [torch.zeros((8,) + tuple(w.grid_shape), dtype=torch.complex64).pin_memory() for _ in range(3)]
+    with pytest.raises(das.DasError):
+        plan.beamform_host_wait()                                # nothing outstanding
+    plan.beamform_host_begin(h_raw[0].data_ptr(), h_out[0].data_ptr())
+    plan.beamform_host_begin(h_raw[1].data_ptr(), h_out[1].data_ptr())
+    with pytest.raises(das.DasError):
+        plan.beamform_host_begin(h_raw[2].data_ptr(), h_out[2].data_ptr())   # a third call in flight
+    with pytest.raises(das.DasError):
+        plan.beamform_host(h_raw[2].data_ptr(), h_out[2].data_ptr())         # the blocking call while calls are outstanding
+    plan.beamform_host_wait()
+    np.testing.assert_array_equal(h_out[0].numpy(), want[0])
+    plan.beamform_host_begin(h_raw[2].data_ptr(), h_out[2].data_ptr())
+    plan.beamform_host_wait()
+    np.testing.assert_array_equal(h_out[1].numpy(), want[1])
+    plan.beamform_host_wait()
+    np.testing.assert_array_equal(h_out[2].numpy(), want[2])
+    plan.destroy()
