@@ -25,8 +25,10 @@ namespace {
 // State of one generator warp: the A slots of its voxel group in tensor memory (das_tc.cuh).
 struct TcGenState {
   unsigned a_addr0;     // TMEM address of slot 0 for this warp's lane quarter
+  unsigned tbl0;        // shared-memory address of row r = 0 of the placement table
   unsigned af0, ae0;    // a_full / a_empty barrier of slot 0 of the group (shared-memory addresses)
   unsigned pend;        // a_full barrier of the item tile whose store is in flight (the sink while there is none)
+  unsigned pend2;       // the same for the overflow tile
   unsigned sink;
   unsigned par;         // bit s: phase parity of the next use of slot s (bit kTcOvf: the overflow slot)
   unsigned it;          // item tiles stored so far (slot = it mod 4 when the transmit count is not 16)
@@ -34,23 +36,32 @@ struct TcGenState {
   unsigned long long pf1, pf2, pf3;
 #endif
   bool free_next;       // the next item's slot was seen free by the probe issued one item ahead
-  bool ovf_pend;        // an overflow tile's store is in flight
-  bool lane0;
 };
 
-// One (q, m) item of a generator thread: the two packed weights, the slot of sample k, the passes.
-struct TcItem { unsigned w0, w1; int r, n_pass; };
+// One (q, m) item of a generator thread: the two packed weights, the shared-memory address of the placement-table row of
+// slot r (sample k sits in slot r of the item's window), the passes.
+struct TcItem { unsigned w0, w1, ra; int n_pass; };
 
-// The A row of one MMA pass: slot r holds W0, slot r + 1 holds W1, every other slot 0 (r in [-1, 7]).
-__device__ __forceinline__ void tc_place(const int r, const unsigned w0, const unsigned w1, unsigned (&v)[8]) {
+// The A row of one MMA pass: slot r holds W0, slot r + 1 holds W1, every other slot 0.  `ra` addresses row r of the
+// placement table (das_tc.cuh): 9 words, word j = {1,1} iff r == j - 1, so slot i = W0 * word[i + 1] + W1 * word[i].
+// The loads are plain (non-volatile) asm: the table never changes, so they may be scheduled across the barrier operations.
+__device__ __forceinline__ void tc_place(const unsigned ra, const unsigned w0, const unsigned w1, unsigned (&v)[8]) {
+#ifdef DAS_TC_WHATIF_PLACE0
+  v[0] = w0; v[1] = w1;
 #pragma unroll
-  for (int i = 0; i < 8; ++i) v[i] = 0u;
+  for (int i = 2; i < 8; ++i) v[i] = ra & 0u;
+#else
+  unsigned t[9];
+  asm("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(t[0]), "=r"(t[1]), "=r"(t[2]), "=r"(t[3]) : "r"(ra));
+  asm("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4+16];" : "=r"(t[4]), "=r"(t[5]), "=r"(t[6]), "=r"(t[7]) : "r"(ra));
+  asm("ld.shared.u32 %0, [%1+32];" : "=r"(t[8]) : "r"(ra));
 #pragma unroll
-  for (int i = -1; i < 8; ++i) {                               // 9 compares, 16 selects
-    const bool hit = r == i;
-    if (i >= 0) v[i] = hit ? w0 : v[i];
-    if (i < 7) v[i + 1] = hit ? w1 : v[i + 1];
+  for (int i = 0; i < 8; ++i) {
+    unsigned m;
+    asm("mul.rn.f16x2 %0, %1, %2;" : "=r"(m) : "r"(w1), "r"(t[i]));
+    asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(v[i]) : "r"(w0), "r"(t[i + 1]), "r"(m));
   }
+#endif
 }
 
 // One NON-BLOCKING probe of an mbarrier phase (test_wait: a scoreboarded read, unlike try_wait, which
@@ -67,54 +78,40 @@ __device__ __forceinline__ unsigned lds_volatile(unsigned addr) {
   asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
   return v;
 }
-// mbarrier arrive under a predicate (no branch: the warp stays converged for the .sync.aligned tcgen05 ops)
-__device__ __forceinline__ void mbar_arrive_if(unsigned bar, bool pred) {
-  asm volatile("{\n\t.reg .pred p;\n\t.reg .b64 st;\n\tsetp.ne.b32 p, %1, 0;\n\t@p mbarrier.arrive.shared::cta.b64 st, [%0];\n\t}"
-               ::"r"(bar), "r"((unsigned)pred) : "memory");
-}
-
-// Third pass of an item (rare: very wide windows), kept out of line.  The overflow tile of the second pass
-// has to be consumed first, and the issuer takes the item tile before it: both stores are completed here,
-// then the overflow slot is reused.  Returns the updated parity word; the caller resets `pend`.
-static __device__ __noinline__ unsigned tc_third_pass(int r, unsigned w0, unsigned w1, unsigned pend, unsigned af0, unsigned ae0,
-                                                      unsigned a_addr0, unsigned par, bool lane0) {
-  unsigned v[8];
-  tc_place(r, w0, w1, v);                                     // r = 8: an all-zero row
-  tmem_wait_st();
-  tc_fence_before();
-  mbar_arrive_if(pend, lane0);
-  mbar_arrive_if(af0 + 8u * kTcOvf, lane0);
-  mbar_wait_park(ae0 + 8u * kTcOvf, ((par >> kTcOvf) & 1u) ^ 1u);
-  tc_fence_after();
-  tmem_st8(a_addr0 + kTcOvf * kTcACols, v);
-  return par ^ (1u << kTcOvf);
+// Two mbarrier arrivals by ONE elected lane of the (converged) warp: the a_full barriers of the item tile and of the
+// overflow tile whose stores have just been seen complete (the sink barrier when there is none).
+__device__ __forceinline__ void mbar_arrive2_elect(unsigned bar0, unsigned bar1) {
+  asm volatile("{\n\t.reg .pred p;\n\t.reg .b64 st;\n\telect.sync _|p, 0xffffffff;\n\t"
+               "@p mbarrier.arrive.shared::cta.b64 st, [%0];\n\t@p mbarrier.arrive.shared::cta.b64 st, [%1];\n\t}"
+               ::"r"(bar0), "r"(bar1) : "memory");
 }
 
 // Hand item I of the current receiver to the MMA issuer.  With 16 transmits per receiver (Q16) the slot
 // S = I mod 4 and the barrier phases are compile-time constants.  Order of events:
-//   placement of this item | completion of the PREVIOUS item's stores (they have had the placement to land)
-//   | slot S free? (probed one item ahead) | store | probe of the next item's slot | overflow pass.
+//   placement of this item | completion of the PREVIOUS item's stores (they have had the placement to land) and
+//   their publication | slot S free? (probed one item ahead) | store | probe of the next item's slot.
+// The second pass of a wide window (13 % of the items at the headline) goes through the overflow slot on a path of
+// its own, so that a one-pass item pays nothing for it.
 template <bool ZERO, bool Q16, int I>
 __device__ __forceinline__ void tc_gen_item(const TcItem& cur, TcGenState& st) {
   const unsigned S = Q16 ? (unsigned)(I & (kTcSlots - 1)) : (st.it & (unsigned)(kTcSlots - 1));
   const unsigned pe = Q16 ? (unsigned)(((I / kTcSlots) & 1) ^ 1) : (((st.par >> S) & 1u) ^ 1u);
-  bool ovf_free = false;
-  if (cur.n_pass > 1) ovf_free = mbar_test(st.ae0 + 8u * kTcOvf, ((st.par >> kTcOvf) & 1u) ^ 1u);
   unsigned v[8];
-  if (!ZERO) tc_place(cur.r, cur.w0, cur.w1, v);
+  if (!ZERO) tc_place(cur.ra, cur.w0, cur.w1, v);
 #ifdef DAS_TC_PROF
   { const long long c0_ = clock64(); tmem_wait_st(); st.pf3 += (unsigned long long)(clock64() - c0_); }
 #else
   tmem_wait_st();
 #endif
   tc_fence_before();
-  mbar_arrive_if(st.pend, st.lane0);
-  mbar_arrive_if(st.af0 + 8u * kTcOvf, st.lane0 && st.ovf_pend);
-  st.ovf_pend = false;
+  mbar_arrive2_elect(st.pend, st.pend2);
+  st.pend2 = st.sink;
 #ifdef DAS_TC_PROF
   if (!st.free_next) { const long long c0_ = clock64(); mbar_wait_park(st.ae0 + 8u * S, pe); st.pf1 += (unsigned long long)(clock64() - c0_); }
 #else
+#ifndef DAS_TC_WHATIF_NOEMPTY
   if (!st.free_next) mbar_wait_park(st.ae0 + 8u * S, pe);
+#endif
 #endif
   tc_fence_after();
   if (ZERO) tmem_st8_zero(st.a_addr0 + S * kTcACols); else tmem_st8(st.a_addr0 + S * kTcACols, v);
@@ -127,21 +124,19 @@ __device__ __forceinline__ void tc_gen_item(const TcItem& cur, TcGenState& st) {
     st.free_next = mbar_test(st.ae0 + 8u * Sn, pn);
   }
   if (cur.n_pass > 1) {
-    // the second pass of the window goes through the overflow slot (uniform branch, ~30 % of the items)
-    if (!ZERO) tc_place(cur.r - kTcBlk * kTcPassBlocks, cur.w0, cur.w1, v);
+    if (!ZERO) tc_place(cur.ra - (unsigned)(kTcPass * kTcPlaceWords * 4), cur.w0, cur.w1, v);
+    const unsigned po = ((st.par >> kTcOvf) & 1u) ^ 1u;
 #ifdef DAS_TC_PROF
-    if (!ovf_free) { const long long c0_ = clock64(); mbar_wait_park(st.ae0 + 8u * kTcOvf, ((st.par >> kTcOvf) & 1u) ^ 1u); st.pf2 += (unsigned long long)(clock64() - c0_); }
+    if (!mbar_test(st.ae0 + 8u * kTcOvf, po)) { const long long c0_ = clock64(); mbar_wait_park(st.ae0 + 8u * kTcOvf, po); st.pf2 += (unsigned long long)(clock64() - c0_); }
 #else
-    if (!ovf_free) mbar_wait_park(st.ae0 + 8u * kTcOvf, ((st.par >> kTcOvf) & 1u) ^ 1u);
+#ifndef DAS_TC_WHATIF_NOEMPTY
+    if (!mbar_test(st.ae0 + 8u * kTcOvf, po)) mbar_wait_park(st.ae0 + 8u * kTcOvf, po);
+#endif
 #endif
     st.par ^= 1u << kTcOvf;
     tc_fence_after();
     if (ZERO) tmem_st8_zero(st.a_addr0 + kTcOvf * kTcACols); else tmem_st8(st.a_addr0 + kTcOvf * kTcACols, v);
-    if (cur.n_pass > 2) {
-      st.par = tc_third_pass(ZERO ? 8 : cur.r - 2 * kTcBlk * kTcPassBlocks, cur.w0, cur.w1, st.pend, st.af0, st.ae0, st.a_addr0, st.par, st.lane0);
-      st.pend = st.sink;
-    }
-    st.ovf_pend = true;
+    st.pend2 = st.af0 + 8u * kTcOvf;
   }
 }
 
@@ -155,7 +150,7 @@ __device__ __forceinline__ void tc_gen_item(const TcItem& cur, TcGenState& st) {
 // phases are compile-time constants.  Tf2 / pc2 / ps2: (q = 2 j, q = 2 j + 1).
 template <bool EDGE, bool ZERO, bool Q16>
 __device__ __forceinline__ void tc_gen_receiver(const float2 (&Tf2)[8], const float2 (&pc2)[8], const float2 (&ps2)[8],
-                                                const float ex, const float pr, const float pi, const uint4 cw0,
+                                                const float ex, const float pr, const float pi, const unsigned am, const uint4 cw0,
                                                 const uint4 cw1, const int tb_l, const int Q, const int K, TcGenState& st) {
   const unsigned cw[8] = {cw0.x, cw0.y, cw0.z, cw0.w, cw1.x, cw1.y, cw1.z, cw1.w};
   const float2 ex2 = make_float2(ex, ex), pr2 = make_float2(pr, pr), npr2 = make_float2(-pr, -pr);
@@ -171,8 +166,9 @@ __device__ __forceinline__ void tc_gen_receiver(const float2 (&Tf2)[8], const fl
     const float2 u = __fadd2_rn(__fadd2_rn(t, mh2), mg2);
     const float2 al = __ffma2_rn(__fadd2_rn(u, nmg2), make_float2(-1.f, -1.f), t);
     // slot of sample k inside the item's window:  r = ki - window start
-    i0.r = (int)__float_as_uint(u.x) - (int)(kMagicBits + (unsigned)code_start(c0));
-    i1.r = (int)__float_as_uint(u.y) - (int)(kMagicBits + (unsigned)code_start(c1));
+    // (a thread outside the aperture has zero weights and an arbitrary index: `am` = 0 sends it to row 0)
+    i0.ra = st.tbl0 + (unsigned)(kTcPlaceWords * 4) * ((__float_as_uint(u.x) - (kMagicBits + (unsigned)code_start(c0))) & am);
+    i1.ra = st.tbl0 + (unsigned)(kTcPlaceWords * 4) * ((__float_as_uint(u.y) - (kMagicBits + (unsigned)code_start(c1))) & am);
     // weights: P = Ptx_q Prx_m;  W1 = al P (sample k + 1),  W0 = P - W1 (sample k); the imaginary parts
     // are carried negated (the A row holds (Re W, -Im W))
     const float2 wre = __ffma2_rn(pc2[jp], pr2, __fmul2_rn(ps2[jp], npi2));          //  Re P
@@ -191,7 +187,7 @@ __device__ __forceinline__ void tc_gen_receiver(const float2 (&Tf2)[8], const fl
     }
   };
   TcItem c0, c1;
-  c0.w0 = c0.w1 = c1.w0 = c1.w1 = 0u; c0.r = c1.r = 0;
+  c0.w0 = c0.w1 = c1.w0 = c1.w1 = 0u; c0.ra = c1.ra = st.tbl0;
   item_pair(0, c0, c1);
 #define DAS_TC_PAIR(JP)                                                        \
   {                                                                            \
@@ -235,14 +231,16 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
   asm volatile("mov.u32 %0, %1;" : "=r"(sinkb) : "r"(smem_u32(&sm.sink)));
 
   if (tid == 0) {
-    for (int s = 0; s < kTcMaxStages; ++s) { mbar_init(b_full0 + 8 * s, 1); mbar_init(b_empty0 + 8 * s, kTcG * kTcIss); }
+    for (int s = 0; s < kTcMaxStages; ++s) { mbar_init(b_full0 + 8 * s, 1); mbar_init(b_empty0 + 8 * s, kTcG); }
     for (int i = 0; i < kTcABufs * kTcG; ++i) { mbar_init(a_full0 + 8 * i, 4); mbar_init(a_empty0 + 8 * i, 1); }
-    mbar_init(d_full, kTcG * kTcIss);
+    mbar_init(d_full, kTcG);
     mbar_init(d_empty, kTcGenWarps);
     mbar_init(sinkb, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == kTcGenWarps) tmem_alloc(smem_u32(&sm.tmem_base), kTcTmemCols);
+  for (int i = tid; i < kTcPlaceRows * kTcPlaceWords; i += kTcThreads)
+    sm.place[i / kTcPlaceWords][i % kTcPlaceWords] = (i / kTcPlaceWords + kTcPlaceLo == i % kTcPlaceWords - 1) ? 0x3C003C00u : 0u;
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -294,14 +292,18 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
           if (code_passes(c[g])) { lo = min(lo, code_start(c[g])); used = true; r.big = r.big || (c[g] & kTcCodeBig); }
         }
         if (!used) lo = 0;
-        // info word: passes | K-row offset of the group's window inside the box (16-byte units) << 2 | big box << 30
+        // info word: K-row offset of the group's window inside the box (16-byte units; the stage slot's address is
+        // added when the word is published) | passes << 14 | big box << 16
 #pragma unroll
         for (int g = 0; g < kTcG; ++g)
-          r.inf[g] = has_q ? ((unsigned)code_passes(c[g]) | ((code_passes(c[g]) ? (unsigned)(2 * (code_start(c[g]) - lo)) : 0u) << 2) |
-                              (r.big ? 0x40000000u : 0u)) : 0u;
+          r.inf[g] = has_q ? (((unsigned)code_passes(c[g]) << 14) | (code_passes(c[g]) ? (unsigned)(2 * (code_start(c[g]) - lo)) : 0u) |
+                              (r.big ? 0x10000u : 0u)) : 0u;
         r.bytes = (has_q && used) ? (r.big ? stage_bytes : small_bytes) : 0u;
         r.c0 = 8 * (tb_q + lo);                               // 32-bit elements: 4 per K row, 2 K rows per sample
         r.c2 = (chunk * P.M + (int)hd.x) * P.Q + ql;
+#ifdef DAS_TC_WHATIF_SAMEBOX
+        r.c2 = ql; r.c0 = 8 * 64;
+#endif
         return r;
       };
       // index of the last list entry any group uses (its last stage ends the tile for the issuers)
@@ -336,9 +338,10 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
           TC_PROF_WAIT(1, if (lane == 0) mbar_wait_park(b_empty0 + 8 * s, ph ^ 1u); __syncwarp())
           __syncwarp();
           if (mine) {
+            const unsigned slot_u16 = (stage0 + (s * qs + (unsigned)(lane - q0)) * stage_bytes) >> 4;   // the item's window slot
 #pragma unroll
             for (int g = 0; g < kTcG; ++g)
-              sm.info[(s * kTcMaxQs + (unsigned)(lane - q0)) * kTcG + g] = cur.inf[g] | ((last_stage && lane == q0) ? 0x80000000u : 0u);
+              sm.info[(s * kTcMaxQs + (unsigned)(lane - q0)) * kTcG + g] = (cur.inf[g] + slot_u16) | ((last_stage && lane == q0) ? 0x80000000u : 0u);
           }
           __syncwarp();
           if (lane == 0) {
@@ -354,7 +357,7 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
       }
     }
     TC_PROF_END
-  } else if (warp > kTcGenWarps + kTcIss * kTcG) {
+  } else if (warp > kTcGenWarps + kTcG) {
     reg_dec<kTcRegsSvc>();                                   // idle warp (roles come in whole warpgroups: setmaxnreg)
   } else if (warp > kTcGenWarps) {
     reg_dec<kTcRegsSvc>();
@@ -365,66 +368,61 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
     // same scalar loop (no divergence, one shuffle per item), only the tcgen05 instructions sit
     // under an elected lane, and the stage barriers are visited once per qs items.  Item q takes
     // its A tile from slot q mod 4, further passes from the overflow slot (das_tc.cuh).
-    const int g = (warp - kTcGenWarps - 1) / kTcIss;
-    const unsigned turn = (unsigned)((warp - kTcGenWarps - 1) % kTcIss);   // this warp issues the items with n_main mod kTcIss == turn
-    if (lane == 0) {
+    const int g = warp - kTcGenWarps - 1;
+    {
       const unsigned idesc = tc_idesc(N);
       const unsigned d_tmem = tmem + (unsigned)(g * N);
       const unsigned a_tmem0 = tmem + a_col0 + (unsigned)(kTcABufs * g) * kTcACols;
       const unsigned af0 = a_full0 + 8u * (unsigned)(kTcABufs * g), ae0 = a_empty0 + 8u * (unsigned)(kTcABufs * g);
-      // descriptor of a B tile at shared address 0: LBO = 8 K rows (the next core matrix along K), SBO = one
-      // column group of the box (its K rows: small or big box); only the 14-bit address field (bits 0-13 of the low
-      // word, 16-byte units = K rows) changes from MMA to MMA
+      // descriptor of a B tile: LBO = 8 K rows (the next core matrix along K), SBO = one column group of the box (its K
+      // rows: small or big box); the 14-bit start address (16-byte units = K rows) comes ready-made from the producer
       const unsigned long long desc_s = tc_smem_desc(0u, 8 * 16, 2 * kTcBoxSmall * 16), desc_b = tc_smem_desc(0u, 8 * 16, 2 * kTcBoxBig * 16);
       const unsigned desc_lo0 = (unsigned)desc_s, desc_hi_s = (unsigned)(desc_s >> 32), desc_hi_b = (unsigned)(desc_b >> 32);
-      const unsigned stage_u16 = stage_bytes >> 4, pass_u16 = 2 * kTcPass;   // K rows of one MMA pass
       const unsigned info0 = smem_u32(&sm.info[0]) + 4u * (unsigned)g;
-      // n_main / n_ovf: MMAs issued so far from item tiles / overflow tiles.  Item tiles use their 4 slots
-      // round robin, so slot and barrier phase follow from the counter: slot = n mod 4, parity = (n / 4) mod 2.
-      unsigned s = 0, ph = 0, n_done = 0, n_main = 0, n_ovf = 0;
+      // Item tiles use their 4 slots round robin: aoff = 8 * slot is the byte offset of the slot's barriers and its
+      // column offset in tensor memory; apar / opar = phase parity of the next use of the item slots / the overflow slot
+      unsigned s = 0, ph = 0, n_done = 0, aoff = 0, apar = 0, opar = 0;
       TC_PROF_DECL
       for (int work = blockIdx.x; work < n_work; work += gridDim.x, ++n_done) {
         TC_PROF_WAIT(1, mbar_wait_park(d_empty, (n_done & 1u) ^ 1u))           // epilogue of the previous tile has drained D
         tc_fence_after();
         bool last = false;
         while (!last) {
-          TC_PROF_WAIT(2, mbar_wait_park(b_full0 + 8 * s, ph))
-          unsigned slot_u16 = (stage0 + s * qs * stage_bytes) >> 4;       // window slot of the item, 16-byte units
+          TC_PROF_WAIT(2, if (!mbar_test(b_full0 + 8 * s, ph)) mbar_wait_park(b_full0 + 8 * s, ph))
           unsigned ia = info0 + s * (kTcMaxQs * kTcG * 4u);
           unsigned info = lds_volatile(ia);
           last = (info >> 31) != 0u;
-          info &= 0x7fffffffu;
-          for (unsigned i = 0; i < qs; ++i, slot_u16 += stage_u16) {
+          for (unsigned i = 0; i < qs; ++i) {
             ia += kTcG * 4u;
             const unsigned info_next = (i + 1 < qs) ? lds_volatile(ia) : 0u;   // one item ahead (slots beyond Q hold 0)
-            const unsigned np = info & 3u;
-            if (np && n_main % kTcIss != turn) {
-              n_ovf += np - 1u;
-              ++n_main;
-            } else if (np) {
-              const unsigned sl = n_main & (kTcSlots - 1);
-              unsigned dlo = desc_lo0 + slot_u16 + ((info >> 2) & 0xfffu);
-              const unsigned desc_hi = (info & 0x40000000u) ? desc_hi_b : desc_hi_s;
-              TC_PROF_WAIT(3, mbar_wait_park(af0 + 8u * sl, (n_main >> 2) & 1u))
+            const unsigned np = (info >> 14) & 3u;
+            if (np) {
+              const unsigned dlo = desc_lo0 | (info & 0x3fffu);
+              const unsigned dhi = (info & 0x10000u) ? desc_hi_b : desc_hi_s;
+#ifndef DAS_TC_WHATIF_NOFULL
+              TC_PROF_WAIT(3, if (!mbar_test(af0 + aoff, apar)) mbar_wait_park(af0 + aoff, apar))
+#endif
               tc_fence_after();
-              TC_PROF_WAIT(5, tc_mma_ts(d_tmem, a_tmem0 + sl * kTcACols, ((unsigned long long)desc_hi << 32) | dlo, idesc, 1u))
-              TC_PROF_WAIT(6, tc_commit(ae0 + 8u * sl))                        // completes when this MMA has read its A slot
-              for (unsigned p = 1; p < np; ++p) {
-                dlo += pass_u16;
-                TC_PROF_WAIT(4, mbar_wait_park(af0 + 8u * kTcOvf, n_ovf & 1u))
-                ++n_ovf;
+              tc_mma_commit(d_tmem, a_tmem0 + aoff, dlo, dhi, idesc, ae0 + aoff);   // the commit completes when the MMA has read its A slot
+              if (np > 1) {
+#ifndef DAS_TC_WHATIF_NOFULL
+                TC_PROF_WAIT(4, if (!mbar_test(af0 + 8u * kTcOvf, opar)) mbar_wait_park(af0 + 8u * kTcOvf, opar))
+#endif
+                opar ^= 1u;
                 tc_fence_after();
-                tc_mma_ts(d_tmem, a_tmem0 + kTcOvf * kTcACols, ((unsigned long long)desc_hi << 32) | dlo, idesc, 1u);
-                tc_commit(ae0 + 8u * kTcOvf);
+                tc_mma_commit(d_tmem, a_tmem0 + kTcOvf * kTcACols, dlo + 2u * kTcPass, dhi, idesc, ae0 + 8u * kTcOvf);
               }
-              ++n_main;
+              aoff = (aoff + 8u) & (8u * kTcSlots - 1u);
+              apar ^= (aoff == 0u) ? 1u : 0u;
             }
             info = info_next;
           }
-          tc_commit(b_empty0 + 8 * s);                         // this group is done with the stage
+          if (tc_elect()) tc_commit(b_empty0 + 8 * s);         // this group is done with the stage
+          __syncwarp();
           if (++s == (unsigned)tp.n_stages) { s = 0; ph ^= 1u; }
         }
-        tc_commit(d_full);                                     // this group's MMAs of the tile are complete
+        if (tc_elect()) tc_commit(d_full);                     // this group's MMAs of the tile are complete
+        __syncwarp();
       }
       TC_PROF_END
     }
@@ -439,13 +437,13 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
     asm volatile("mov.u32 %0, %1;" : "=r"(st.a_addr0) : "r"(tmem + lane_base + a_col0 + (unsigned)(kTcABufs * g) * kTcACols));
     asm volatile("mov.u32 %0, %1;" : "=r"(st.ae0) : "r"(a_empty0 + 8u * (unsigned)(kTcABufs * g)));
     asm volatile("mov.u32 %0, %1;" : "=r"(st.af0) : "r"(a_full0 + 8u * (unsigned)(kTcABufs * g)));
+    asm volatile("mov.u32 %0, %1;" : "=r"(st.tbl0) : "r"(smem_u32(&sm.place[-kTcPlaceLo][0])));
     st.sink = sinkb;
     st.pend = sinkb;
+    st.pend2 = sinkb;
     st.it = 0u;
     st.par = 0u;
     st.free_next = false;
-    st.ovf_pend = false;
-    st.lane0 = lane == 0;
     unsigned n_done = 0;
     TC_PROF_DECL
 #ifdef DAS_TC_PROF
@@ -497,14 +495,17 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
           if (P.has_dir) dir_n = __ldg(&P.edir[hd_n.x]);
         }
         if (!((hd.y >> g) & 1u)) continue;                    // no voxel of this group sees receiver m
+#ifdef DAS_TC_WHATIF_GEN_IDLE
+        continue;
+#endif
         // per-(m, n): aperture, excess path, receive phase (as in das_tiled.cuh)
         bool act;
         float wrx;
         const float ex = tc_excess(tp, P, vx, el, dir, act, wrx);
         if (!__any_sync(0xffffffffu, act)) {
           // no voxel of this WARP sees the receiver: 32 zero rows per item, no arithmetic
-          if (q16) tc_gen_receiver<false, true, true>(Tf, pc, ps, 0.f, 0.f, 0.f, cw0, cw1, tb_l, P.Q, P.K, st);
-          else tc_gen_receiver<false, true, false>(Tf, pc, ps, 0.f, 0.f, 0.f, cw0, cw1, tb_l, P.Q, P.K, st);
+          if (q16) tc_gen_receiver<false, true, true>(Tf, pc, ps, 0.f, 0.f, 0.f, 0u, cw0, cw1, tb_l, P.Q, P.K, st);
+          else tc_gen_receiver<false, true, false>(Tf, pc, ps, 0.f, 0.f, 0.f, 0u, cw0, cw1, tb_l, P.Q, P.K, st);
           continue;
         }
         float cyc = tp.ratio_f * ex;
@@ -512,19 +513,18 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
         const float ang = 6.283185307179586f * cyc;
         const float pr = act ? wrx * cos_approx(ang) : 0.f, pi = act ? wrx * sin_approx(ang) : 0.f;
         if (q16) {
-          if (td.edge) tc_gen_receiver<true, false, true>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, st);
-          else tc_gen_receiver<false, false, true>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, st);
+          if (td.edge) tc_gen_receiver<true, false, true>(Tf, pc, ps, ex, pr, pi, act ? 0xffffffffu : 0u, cw0, cw1, tb_l, P.Q, P.K, st);
+          else tc_gen_receiver<false, false, true>(Tf, pc, ps, ex, pr, pi, act ? 0xffffffffu : 0u, cw0, cw1, tb_l, P.Q, P.K, st);
         } else {
-          if (td.edge) tc_gen_receiver<true, false, false>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, st);
-          else tc_gen_receiver<false, false, false>(Tf, pc, ps, ex, pr, pi, cw0, cw1, tb_l, P.Q, P.K, st);
+          if (td.edge) tc_gen_receiver<true, false, false>(Tf, pc, ps, ex, pr, pi, act ? 0xffffffffu : 0u, cw0, cw1, tb_l, P.Q, P.K, st);
+          else tc_gen_receiver<false, false, false>(Tf, pc, ps, ex, pr, pi, act ? 0xffffffffu : 0u, cw0, cw1, tb_l, P.Q, P.K, st);
         }
       }
       tmem_wait_st();
       tc_fence_before();
-      mbar_arrive_if(st.pend, st.lane0);
-      mbar_arrive_if(st.af0 + 8u * kTcOvf, st.lane0 && st.ovf_pend);
+      mbar_arrive2_elect(st.pend, st.pend2);
       st.pend = sinkb;
-      st.ovf_pend = false;
+      st.pend2 = sinkb;
 
       // ---- epilogue: D (FP32, TMEM) -> out[frame][voxel] -------------------------------------
       TC_PROF_WAIT(3, mbar_wait_park(d_full, n_done & 1u))

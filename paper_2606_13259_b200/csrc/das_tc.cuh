@@ -68,16 +68,19 @@ constexpr int kTcMaxStages = 16;            // upper bound of the shared-memory 
 constexpr int kTcMinStages = 2;
 constexpr int kTcMaxQs = 16;                // upper bound of the window slots (transmits) per stage
 constexpr int kTcGenWarps = 4 * kTcG;
-constexpr int kTcIss = 2;                    // MMA issuer warps per voxel group: the issue chain of one warp
-                                             // (~45 instructions per MMA at single-warp latency) caps a group
-                                             // at one MMA per ~400 cycles; the issuers take the items in turn
-constexpr int kTcSvcWarps = 8;               // TMA producer + kTcIss issuers per voxel group (+ idle: whole warpgroups)
+constexpr int kTcSvcWarps = 4;               // TMA producer + one MMA issuer per voxel group (whole warpgroups: setmaxnreg)
 constexpr int kTcThreads = (kTcSvcWarps + kTcGenWarps) * 32;
-constexpr int kTcRegsGen = 128, kTcRegsSvc = 40;   // setmaxnreg: 12 x 32 x 128 + 8 x 32 x 40 <= 65536
-static_assert(1 + kTcIss * kTcG <= kTcSvcWarps && kTcSvcWarps % 4 == 0 && kTcGenWarps % 4 == 0, "warpgroup roles");
+constexpr int kTcRegsGen = 128, kTcRegsSvc = 40;   // setmaxnreg: the service warps hand their registers back
+static_assert(1 + kTcG <= kTcSvcWarps && kTcSvcWarps % 4 == 0 && kTcGenWarps % 4 == 0, "warpgroup roles");
 constexpr int kTcTmemCols = 512;
 constexpr int kTcACols = 8;                 // TMEM columns of one A buffer (K = 16 FP16 per row)
 constexpr float kTcMargin = 0.02f;          // samples: slack of the plan's transmit-delay bounds (tbase)
+// Placement table (shared memory): row r (r = slot of sample k inside the MMA pass, kTcPlaceLo <= r <= kTcPlaceHi) holds
+// the FP16x2 factors {1,1} / {0,0} that put W0 into slot r and W1 into slot r + 1 of the 8-slot A row: word j of a row
+// is 1 iff r == j - 1.  A generator thread loads the 9 words of its row and forms slot i as W0 * word[i + 1] + W1 * word[i]
+// (HMUL2 + HFMA2: the placement runs on the FMA pipe instead of 9 compares + 16 selects on the half-rate ALU pipe).
+constexpr int kTcPlaceLo = -9, kTcPlaceHi = 16, kTcPlaceWords = 12;
+constexpr int kTcPlaceRows = kTcPlaceHi - kTcPlaceLo + 1;
 
 
 struct TcTile {
@@ -255,6 +258,7 @@ struct alignas(128) TcSmemHeader {
   unsigned long long d_full, d_empty;
   unsigned long long sink;           // arrivals nobody waits for (no A tile in flight)
   unsigned info[kTcMaxStages * kTcMaxQs * kTcG];   // per stage and window slot: what each group's issuer does with the item
+  alignas(16) unsigned place[kTcPlaceRows][kTcPlaceWords];   // placement table (see kTcPlaceLo)
   unsigned tmem_base;
 };
 
