@@ -46,11 +46,6 @@ struct TcItem { unsigned w0, w1, ra; int n_pass; };
 // placement table (das_tc.cuh): 9 words, word j = {1,1} iff r == j - 1, so slot i = W0 * word[i + 1] + W1 * word[i].
 // The loads are plain (non-volatile) asm: the table never changes, so they may be scheduled across the barrier operations.
 __device__ __forceinline__ void tc_place(const unsigned ra, const unsigned w0, const unsigned w1, unsigned (&v)[8]) {
-#ifdef DAS_TC_WHATIF_PLACE0
-  v[0] = w0; v[1] = w1;
-#pragma unroll
-  for (int i = 2; i < 8; ++i) v[i] = ra & 0u;
-#else
   unsigned t[9];
   asm("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(t[0]), "=r"(t[1]), "=r"(t[2]), "=r"(t[3]) : "r"(ra));
   asm("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4+16];" : "=r"(t[4]), "=r"(t[5]), "=r"(t[6]), "=r"(t[7]) : "r"(ra));
@@ -61,7 +56,6 @@ __device__ __forceinline__ void tc_place(const unsigned ra, const unsigned w0, c
     asm("mul.rn.f16x2 %0, %1, %2;" : "=r"(m) : "r"(w1), "r"(t[i]));
     asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(v[i]) : "r"(w0), "r"(t[i + 1]), "r"(m));
   }
-#endif
 }
 
 // One NON-BLOCKING probe of an mbarrier phase (test_wait: a scoreboarded read, unlike try_wait, which
@@ -109,9 +103,7 @@ __device__ __forceinline__ void tc_gen_item(const TcItem& cur, TcGenState& st) {
 #ifdef DAS_TC_PROF
   if (!st.free_next) { const long long c0_ = clock64(); mbar_wait_park(st.ae0 + 8u * S, pe); st.pf1 += (unsigned long long)(clock64() - c0_); }
 #else
-#ifndef DAS_TC_WHATIF_NOEMPTY
   if (!st.free_next) mbar_wait_park(st.ae0 + 8u * S, pe);
-#endif
 #endif
   tc_fence_after();
   if (ZERO) tmem_st8_zero(st.a_addr0 + S * kTcACols); else tmem_st8(st.a_addr0 + S * kTcACols, v);
@@ -129,9 +121,7 @@ __device__ __forceinline__ void tc_gen_item(const TcItem& cur, TcGenState& st) {
 #ifdef DAS_TC_PROF
     if (!mbar_test(st.ae0 + 8u * kTcOvf, po)) { const long long c0_ = clock64(); mbar_wait_park(st.ae0 + 8u * kTcOvf, po); st.pf2 += (unsigned long long)(clock64() - c0_); }
 #else
-#ifndef DAS_TC_WHATIF_NOEMPTY
     if (!mbar_test(st.ae0 + 8u * kTcOvf, po)) mbar_wait_park(st.ae0 + 8u * kTcOvf, po);
-#endif
 #endif
     st.par ^= 1u << kTcOvf;
     tc_fence_after();
@@ -258,8 +248,8 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
   __syncthreads();
   tc_fence_after();
 
+  // 512 threads x 128 registers: every role keeps its full share (no setmaxnreg; the service warps spill at 40)
   if (warp == kTcGenWarps) {
-    reg_dec<kTcRegsSvc>();
     // ===================================== TMA PRODUCER =======================================
     // A stage holds the windows of `qs` consecutive transmits of one receiver (one barrier round
     // per qs items).  Lane q works out the window of item (q, m), the union over the voxel groups,
@@ -301,9 +291,6 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
         r.bytes = (has_q && used) ? (r.big ? stage_bytes : small_bytes) : 0u;
         r.c0 = 8 * (tb_q + lo);                               // 32-bit elements: 4 per K row, 2 K rows per sample
         r.c2 = (chunk * P.M + (int)hd.x) * P.Q + ql;
-#ifdef DAS_TC_WHATIF_SAMEBOX
-        r.c2 = ql; r.c0 = 8 * 64;
-#endif
         return r;
       };
       // index of the last list entry any group uses (its last stage ends the tile for the issuers)
@@ -358,16 +345,16 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
     }
     TC_PROF_END
   } else if (warp > kTcGenWarps + kTcG) {
-    reg_dec<kTcRegsSvc>();                                   // idle warp (roles come in whole warpgroups: setmaxnreg)
+    // no role
   } else if (warp > kTcGenWarps) {
-    reg_dec<kTcRegsSvc>();
     // ===================================== MMA ISSUERS ========================================
-    // One warp per voxel group.  The issue loop is a serial chain (wait -> MMA -> commit) whose
-    // latency bounds the MMA rate of a group, so it is kept as short as it can be: lane q prepares
-    // item (q, m) (passes, offset of the group's window inside the staged one), every lane runs the
-    // same scalar loop (no divergence, one shuffle per item), only the tcgen05 instructions sit
-    // under an elected lane, and the stage barriers are visited once per qs items.  Item q takes
-    // its A tile from slot q mod 4, further passes from the overflow slot (das_tc.cuh).
+    // One warp per voxel group.  The issue loop is a serial chain (probe -> MMA -> commit) whose
+    // latency bounds the MMA rate of a group (measured: it, not the generators' instruction count,
+    // set the pace), so it is kept short and small: the producer publishes the ready-made start
+    // address of every window, EVERY lane runs the same loop (a loop under `lane == 0` makes ptxas
+    // wrap each tcgen05 instruction in an elect / broadcast loop), the MMA and its commit sit under
+    // elect.sync inside one asm block, and the stage barriers are visited once per qs items.  Item q
+    // takes its A tile from slot q mod 4, a second pass from the overflow slot (das_tc.cuh).
     const int g = warp - kTcGenWarps - 1;
     {
       const unsigned idesc = tc_idesc(N);
@@ -399,15 +386,11 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
             if (np) {
               const unsigned dlo = desc_lo0 | (info & 0x3fffu);
               const unsigned dhi = (info & 0x10000u) ? desc_hi_b : desc_hi_s;
-#ifndef DAS_TC_WHATIF_NOFULL
               TC_PROF_WAIT(3, if (!mbar_test(af0 + aoff, apar)) mbar_wait_park(af0 + aoff, apar))
-#endif
               tc_fence_after();
               tc_mma_commit(d_tmem, a_tmem0 + aoff, dlo, dhi, idesc, ae0 + aoff);   // the commit completes when the MMA has read its A slot
               if (np > 1) {
-#ifndef DAS_TC_WHATIF_NOFULL
                 TC_PROF_WAIT(4, if (!mbar_test(af0 + 8u * kTcOvf, opar)) mbar_wait_park(af0 + 8u * kTcOvf, opar))
-#endif
                 opar ^= 1u;
                 tc_fence_after();
                 tc_mma_commit(d_tmem, a_tmem0 + kTcOvf * kTcACols, dlo + 2u * kTcPass, dhi, idesc, ae0 + 8u * kTcOvf);
@@ -428,7 +411,6 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
     }
   } else {
     // ===================================== GENERATORS =========================================
-    reg_inc<kTcRegsGen>();
     const int g = warp >> 2;                                  // voxel group = depth inside the tile
     const int row = (warp & 3) * 32 + lane;                   // MMA row = TMEM lane (quarter warp % 4)
     const unsigned lane_base = ((unsigned)((warp & 3) * 32)) << 16;
@@ -495,9 +477,6 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
           if (P.has_dir) dir_n = __ldg(&P.edir[hd_n.x]);
         }
         if (!((hd.y >> g) & 1u)) continue;                    // no voxel of this group sees receiver m
-#ifdef DAS_TC_WHATIF_GEN_IDLE
-        continue;
-#endif
         // per-(m, n): aperture, excess path, receive phase (as in das_tiled.cuh)
         bool act;
         float wrx;

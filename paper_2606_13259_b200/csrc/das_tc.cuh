@@ -35,7 +35,7 @@
 //                item are therefore compile-time constants in the unrolled transmit loop: one
 //                mbarrier round per item with no ring arithmetic.
 //   warp 12      TMA producer: one bulk copy per (q, m) of the k-blocks the tile needs.
-//   warps 13..18 MMA issuers, two per voxel group: tcgen05.mma.kind::f16, A from TMEM, B from
+//   warps 13..15 MMA issuers, one per voxel group: tcgen05.mma.kind::f16, A from TMEM, B from
 //                shared memory, D of the group in TMEM.  B is MN-MAJOR without swizzle: a K row is one
 //                (sample, y | -j y) vector over the N = 2 Bc frame columns, stored as N / 8 column
 //                groups of 16 bytes; per column group the K rows are contiguous, so an MMA window
@@ -70,7 +70,6 @@ constexpr int kTcMaxQs = 16;                // upper bound of the window slots (
 constexpr int kTcGenWarps = 4 * kTcG;
 constexpr int kTcSvcWarps = 4;               // TMA producer + one MMA issuer per voxel group (whole warpgroups: setmaxnreg)
 constexpr int kTcThreads = (kTcSvcWarps + kTcGenWarps) * 32;
-constexpr int kTcRegsGen = 128, kTcRegsSvc = 40;   // setmaxnreg: the service warps hand their registers back
 static_assert(1 + kTcG <= kTcSvcWarps && kTcSvcWarps % 4 == 0 && kTcGenWarps % 4 == 0, "warpgroup roles");
 constexpr int kTcTmemCols = 512;
 constexpr int kTcACols = 8;                 // TMEM columns of one A buffer (K = 16 FP16 per row)
