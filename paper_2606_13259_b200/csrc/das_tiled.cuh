@@ -246,6 +246,7 @@ __device__ __forceinline__ void term(unsigned a, float ts, float2 p1, float2 p2,
 
 // Part 1: wait for the stage, read its meta entry, classify the aperture (exactly inside the
 // guard band).  a2e / band carry "voxel outside the grid" and "no apodization" (see the caller).
+template <bool GEN>
 __device__ __forceinline__ void geo_test(Geo& g, unsigned tab_full0, unsigned meta0, unsigned slot, unsigned phase,
                                          float x, float y, int iz, float a, float a2, float a2e, float band,
                                          const TiledDev& tp, const Params& P) {
@@ -255,26 +256,26 @@ __device__ __forceinline__ void geo_test(Geo& g, unsigned tab_full0, unsigned me
   g.rho2 = fmaf(dx, dx, dy * dy);
   g.e0 = meta.z;
   g.mg = meta.w;
-  if (P.has_dir && P.apod) {
+  if (GEN && P.has_dir && P.apod) {
     // tilted normal: the delays are those of the planar array, only the cone turns with the normal
     const float4 dir = lds128<0>(meta0 + 16 * (kTabStages + kRawStages + slot));     // dir_tab[slot]
     g.act = aperture_dir(x, y, meta.x, meta.y, dx, dy, a, g.rho2, a2, dir, tp.four_f2, a2e >= 0.f, P.zs, iz, tp.z_array, P.fnum, g.u2);
     return;
   }
   const float lhs = tp.four_f2 * g.rho2;
-  g.u2 = lhs * rcp_approx(a2);
+  if (GEN) g.u2 = lhs * rcp_approx(a2);
   g.act = lhs <= a2e;
   if (fabsf(lhs - a2e) <= band) g.act = aperture_exact(x, y, meta.x, meta.y, P.zs, iz, tp.z_array, P.fnum);
 }
 // Part 2 (active lanes): excess path and receive phase.
-template <bool IQ>
+template <bool IQ, bool GEN>
 __device__ __forceinline__ void geo_finish(Geo& g, float a, float a2, const TiledDev& tp, const Params& P) {
   const float s2 = g.rho2 + a2;
   const float d = s2 * rsqrt_approx(s2);
   const float e = (g.rho2 * tp.kappa_f) * rcp_approx(a + d);
   g.ep = e - g.e0;
   // receive window (include/das.h): the boxcar leaves the weight at 1
-  const float wrx = (P.window != DAS_WINDOW_BOXCAR && P.apod) ? rx_window(P.window, P.taper, g.u2) : 1.f;
+  const float wrx = (GEN && P.window != DAS_WINDOW_BOXCAR && P.apod) ? rx_window(P.window, P.taper, g.u2) : 1.f;
   if (IQ) {
     float cyc = tp.ratio_f * e;
     cyc -= rintf(cyc);
@@ -287,7 +288,10 @@ __device__ __forceinline__ void geo_finish(Geo& g, float a, float a2, const Tile
   }
 }
 
-template <int QC, int W, int MODE>
+// GEN: the plan uses a part of the general interface (tilted normals, a smooth receive window, transmit delay / weight
+// tables).  The common case (planar normals, boxcar, analytic transmits) is compiled without it: it costs registers
+// in the receiver loop (the 16-transmit instance spilled with it).
+template <int QC, int W, int MODE, bool GEN>
 __global__ void __launch_bounds__(kTiledThreads, 2)
 tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict__ conv, void* __restrict__ out_v) {
   constexpr bool IQ = ModeTraits<MODE>::iq;
@@ -332,7 +336,7 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
             const float4 el = __ldg(&P.elem[m]);
             mbar_wait(raw_empty0 + 8 * slot, ((seq / kRawStages) & 1u) ^ 1u);
             if (lane == 0) {
-              if (P.has_dir) sm.dir_raw[slot] = __ldg(&P.edir[m]);
+              if (GEN && P.has_dir) sm.dir_raw[slot] = __ldg(&P.edir[m]);
               sm.meta_raw[slot] = make_float4(el.x, el.y, (float)e0, 0.f);
               mbar_arrive_expect_tx(raw_full0 + 8 * slot, (unsigned)(nq * W * EB));
             }
@@ -360,7 +364,7 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
             float4 mt = sm.meta_raw[rs];
             mt.w = kMagic + (float)(ts * NE);
             sm.meta_tab[ts] = mt;
-            if (P.has_dir) sm.dir_tab[ts] = sm.dir_raw[rs];
+            if (GEN && P.has_dir) sm.dir_tab[ts] = sm.dir_raw[rs];
           }
           const unsigned src = raw0 + rs * (NE * EB) + lane * EB, dst = tab0 + ts * (NE * TB) + lane * TB;
 #pragma unroll
@@ -440,7 +444,7 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
 #pragma unroll
       for (int j = 0; j < 2 * QP; ++j) {
         const int q = min(q0 + j, P.Q - 1);
-        const double T = (tx_tau(P, q, n_flat, x, y, z) + a_d / P.c - P.t_start) * P.fs;
+        const double T = ((GEN ? tx_tau(P, q, n_flat, x, y, z) : tx_delay(P.tx[q], x, y, z, P.c)) + a_d / P.c - P.t_start) * P.fs;
         const int k0 = __ldg(&tp.k0tile[(long long)tile_i * P.Q + q]);
         const float tf = (float)(T - (double)k0 - 0.5);
         if (j & 1) Tf[j >> 1].y = tf; else Tf[j >> 1].x = tf;
@@ -455,9 +459,9 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
       // ---- receiver loop ---------------------------------------------------------------
       for (int li = 0; li < td.list_cnt; ++li) {
         Geo g;
-        geo_test(g, tab_full0, meta0, slot, phase, x, y, izc, a, a2, a2e, band, tp, P);
+        geo_test<GEN>(g, tab_full0, meta0, slot, phase, x, y, izc, a, a2, a2e, band, tp, P);
         if (g.act) {
-          geo_finish<IQ>(g, a, a2, tp, P);
+          geo_finish<IQ, GEN>(g, a, a2, tp, P);
           const float2 ep2 = make_float2(g.ep, g.ep), mg2 = make_float2(g.mg, g.mg);
           const float2 p1 = make_float2(g.pr, g.pi), p2 = make_float2(-g.pi, g.pr);
           constexpr int kRow = W * TB;
@@ -488,7 +492,7 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
 #pragma unroll
       for (int j = 0; j < 2 * QP; ++j) {
         if (j < QC && q0 + j < P.Q) {
-          const float wq = tx_weight(P, q0 + j, n_flat);        // transmit weight (1 without a table)
+          const float wq = GEN ? tx_weight(P, q0 + j, n_flat) : 1.f;        // transmit weight (1 without a table)
           if (IQ) {
             const float ang = 6.283185307179586f * sm.cyc[IQ ? j : 0][tid];
             const float cs = wq * cos_approx(ang), sn = wq * sin_approx(ang);
@@ -509,18 +513,20 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
 }
 
 // ---- per-mode launcher, instantiated in das_tiled_inst_*.cu ----------------------------------
-template <int QC, int W, int MODE>
-cudaError_t launch_tiled_inst(const TiledDev& tp, const Params& P, const void* conv, void* out, int grid, cudaStream_t s) {
-  auto k = tiled_kernel<QC, W, MODE>;
+template <int QC, int W, int MODE, bool GEN>
+cudaError_t launch_tiled_gen(const TiledDev& tp, const Params& P, const void* conv, void* out, int grid, cudaStream_t s) {
+  auto k = tiled_kernel<QC, W, MODE, GEN>;
   const size_t smem = sizeof(TiledSmem<QC, W, MODE>);
-  static bool configured = false;        // per instantiation
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  // per launch: the attribute belongs to the (device, context) the plan lives on, and setting it is cheap
+  cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
   k<<<grid, kTiledThreads, smem, s>>>(tp, P, static_cast<const unsigned char*>(conv), out);
   return cudaGetLastError();
+}
+template <int QC, int W, int MODE>
+cudaError_t launch_tiled_inst(const TiledDev& tp, const Params& P, const void* conv, void* out, int grid, cudaStream_t s) {
+  const bool gen = P.has_dir || P.window != DAS_WINDOW_BOXCAR || P.tau_tab != nullptr || P.wtx_tab != nullptr;
+  return gen ? launch_tiled_gen<QC, W, MODE, true>(tp, P, conv, out, grid, s) : launch_tiled_gen<QC, W, MODE, false>(tp, P, conv, out, grid, s);
 }
 
 template <int QC, int MODE>
