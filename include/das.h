@@ -120,8 +120,11 @@ typedef struct {
   int   interp;             /* das_interp_t; CUBIC: general kernel only, one frame per call */
 } das_plan_desc_t;
 
-/* Validates *desc, uploads geometry and small derived tables to desc->device, chooses launch
- * shapes.  On success *out_plan is a new plan (free with das_plan_destroy). */
+/* The problem statement of PAPER.md:29-50 (Eq. 1: delays; Eq. 2: the weighted sum; linear interpolation) and
+ * PAPER.md:99-133 (Alg. 1 "Require": geometry, transmit set, voxel positions) as a plan.  Validates *desc,
+ * uploads geometry and small derived tables to desc->device, chooses kernel and launch shapes (with
+ * n_frames = B >= 8 and IQ data in fp16 storage: per-tile sample windows from a plan-time kernel, about
+ * 1.5 s at the headline size).  On success *out_plan is a new plan (free with das_plan_destroy). */
 das_status_t das_plan_create(const das_plan_desc_t* desc, das_plan_t** out_plan);
 das_status_t das_plan_destroy(das_plan_t* plan);            /* NULL is allowed */
 
@@ -141,9 +144,12 @@ int    das_plan_frames(const das_plan_t* plan);      /* B (>= 1)                
 das_status_t das_convert(const das_plan_t* plan, const void* d_raw, void* d_conv, float scale,
                          void* stream);
 
-/* Beamform one volume per frame (B volumes).
- *   d_conv  device, produced by das_convert with this plan (or a plan with identical
- *           n_tx, n_elem, n_samples, data_kind and storage)
+/* Beamform one volume per frame (B volumes): Eq. 2 with the delays of Eq. 1
+ * and linear interpolation evaluated in-kernel for every voxel, rows a2-a6 of SURVEY.md section 8.
+ *   d_conv  device, produced by das_convert with this plan, or with a plan of the same algo (das_plan_algo),
+ *           n_frames, n_tx, n_elem, n_samples, data_kind and storage: the converted layout depends on all of
+ *           them (DAS_ALGO_TC: batch-inner [chunk][M][Q][column group][2K][8] FP16; else [M][Q][Kp] intervals);
+ *           a buffer converted for another layout is not detected
  *   d_out   device, das_output_bytes() bytes, [B][nx][ny][nz] with z fastest (C order), complex64
  *           (IQ) or float32 (RF); overwritten, not accumulated into; 8-byte aligned */
 das_status_t das_execute(const das_plan_t* plan, const void* d_conv, void* d_out, void* stream);
