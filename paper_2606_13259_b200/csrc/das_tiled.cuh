@@ -40,8 +40,8 @@
 
 namespace das {
 
-constexpr int kRawStages = 4;                   // ring of TMA-staged windows (storage precision)
-constexpr int kTabStages = 4;                   // ring of FP32 line tables the consumers read
+constexpr int kRawStages = 6;                   // ring of TMA-staged windows (storage precision)
+constexpr int kTabStages = 6;                   // ring of FP32 line tables the consumers read
 constexpr int kConvWarps = 3;
 constexpr int kHelperWarps = 4;                 // one warpgroup: producer + converters (+ idle)
 constexpr int kLaneX = 8, kLaneY = 4;          // a consumer warp covers 8 x 4 lateral voxels
@@ -54,6 +54,12 @@ constexpr float kMagic = 12582912.0f;           // 1.5 * 2^23: adding it rounds 
 constexpr unsigned kMagicBits = 0x4B400000u;
 constexpr float kBand = 4e-6f;                  // relative guard band of the FP32 aperture test
 static_assert(kConsumerWarps % 4 == 0 && kHelperWarps == 4 && kConvWarps + 1 <= kHelperWarps, "warpgroup roles");
+// The converter warps take the stages in turn.  Both rings must be a multiple of their number deep, so that a slot is
+// always served by the SAME warp: an mbarrier parity wait cannot tell "round r + 1 complete" from "round r - 1
+// complete", and the bulk copies of different stages complete in any order.  With 3 converters and 4 slots a warp
+// could reach a slot whose previous round (another warp's) was still in flight, fall through the wait, convert a
+// stale window and deadlock the rings (about one launch in fifty of the RF fp32 headline; fixed in round 2).
+static_assert(kRawStages % kConvWarps == 0 && kTabStages % kConvWarps == 0, "a slot belongs to one converter warp");
 
 enum Mode { kIQ32 = 0, kIQ16 = 1, kRF32 = 2, kRF16 = 3, kIQ8 = 4, kRF8 = 5 };
 template <int MODE> struct ModeTraits;   // eb: bytes of a stored (mid, slope) entry; tb: of a table entry
@@ -358,6 +364,7 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
         const unsigned end = seq + (unsigned)(tp.tiles[tile_i].list_cnt * tp.n_chunks);
         for (unsigned s = seq + (cw + kConvWarps - seq % kConvWarps) % kConvWarps; s < end; s += kConvWarps) {
           const unsigned rs = s % kRawStages, ts = s % kTabStages;
+          // (stage s always meets the same converter in its slot: kRawStages is a multiple of kConvWarps, see there)
           mbar_wait(raw_full0 + 8 * rs, (s / kRawStages) & 1u);
           mbar_wait(tab_empty0 + 8 * ts, ((s / kTabStages) & 1u) ^ 1u);
           if (lane == 0) {

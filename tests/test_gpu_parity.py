@@ -387,3 +387,30 @@ def test_count_work_out_of_range(das_lib):
     pairs, terms = plan.count_work()
     plan.destroy()
     assert terms == int(cnt.sum()) and terms < pairs * w.n_tx
+
+
+@pytest.mark.timeout(180)
+def test_tiled_kernel_repeated_launches_do_not_hang(das_lib, monkeypatch):
+    """Regression (round 2): with 3 converter warps over 4-deep rings a converter could fall through the parity wait
+    of a slot whose previous round was still in flight; about one launch in fifty of the RF fp32 headline then
+    deadlocked its mbarrier rings (found with cuda-gdb: all three roles of one CTA parked in try_wait).  The rings
+    are now a multiple of the converter count deep.  Few CTAs walking many tiles made the old hang certain within a
+    few launches, so this runs the RF fp32 headline geometry with 74 CTAs, 40 launches back to back, and compares
+    the last result with the first (the kernel is deterministic)."""
+    torch = _torch()
+    das = das_lib
+    monkeypatch.setenv("DAS_TILED_GRID", "74")
+    w = wl.config(4, generate_data=False)
+    plan = das.Plan.from_workload(w, storage=das.STORE_FP32, algo=das.ALGO_TILED)
+    g = torch.Generator(device="cuda").manual_seed(3)
+    raw = torch.randn((w.n_tx, w.n_elem, w.n_samples), device="cuda", generator=g)
+    conv = torch.empty(plan.converted_bytes, dtype=torch.uint8, device="cuda")
+    outs = [torch.empty(plan.output_bytes // 4, dtype=torch.float32, device="cuda") for _ in range(2)]
+    s = torch.cuda.current_stream().cuda_stream
+    plan.convert(raw.data_ptr(), conv.data_ptr(), 1.0, s)
+    plan.execute(conv.data_ptr(), outs[0].data_ptr(), s)
+    for _ in range(40):
+        plan.execute(conv.data_ptr(), outs[1].data_ptr(), s)
+    torch.cuda.synchronize()
+    assert torch.equal(outs[0], outs[1])
+    plan.destroy()
