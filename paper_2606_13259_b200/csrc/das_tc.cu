@@ -267,11 +267,12 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
       // item (q = lane, m) of a list entry: first K row of its box (the union of the groups' windows), the
       // tensor coordinate of its (m, q) record, and the issuers' info words; fetched one entry ahead (the
       // loads are a dependent chain through L2)
-      struct Ent { unsigned any, bytes, inf[kTcG]; int c0, c2; bool big; };
+      struct Ent { unsigned any, bytes, inf[kTcG], m; int c0, c2; bool big; };
       auto entry_window = [&](const long long e) {
         Ent r;
         const uint2 hd = __ldg(&tp.list[e]);
         r.any = hd.y;
+        r.m = hd.x;
         int lo = 0x7fffffff;
         unsigned c[kTcG];
         bool used = false;
@@ -302,7 +303,7 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
         if (m) last_li = li0 + 31 - __clz(m);
       }
       Ent nx;
-      nx.any = 0; nx.bytes = 0; nx.c0 = 0; nx.c2 = 0; nx.big = false;
+      nx.any = 0; nx.bytes = 0; nx.c0 = 0; nx.c2 = 0; nx.big = false; nx.m = 0;
       if (td.list_cnt) nx = entry_window(td.list_off);
       bool sent = false;
       for (int li = 0; li < td.list_cnt || !sent; ++li) {
@@ -313,17 +314,41 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
           if (!cur.any) continue;
         } else {
           // a tile without any receiver: one empty stage, so that the issuers see the end of the tile
-          cur.any = 0; cur.bytes = 0; cur.c0 = 0; cur.c2 = 0; cur.big = false;
+          cur.any = 0; cur.bytes = 0; cur.c0 = 0; cur.c2 = 0; cur.big = false; cur.m = 0xffffu;
 #pragma unroll
           for (int g = 0; g < kTcG; ++g) cur.inf[g] = 0u;
         }
         sent = true;
+        // ---- quad pacing (L2 reuse) --------------------------------------------------------------------------
+        // CTAs 4 j .. 4 j + 3 work on a 2 x 2 block of laterally adjacent tiles (the plan orders the tiles so), whose
+        // receiver lists and sample windows overlap almost entirely.  Each producer publishes (launch, round, receiver)
+        // before it fetches a receiver's windows and holds back while a partner is more than `pace` receivers behind:
+        // the four then read the same records within microseconds of each other and three of the four reads hit L2.
+        // Advisory only: the wait is bounded, nothing else depends on it.
+        // The partners' words are loaded here and looked at only after the wait for the stage below, so that the
+        // round trip to L2 hides under it; one receiver in four is paced.
+        const bool paced = tp.progress != nullptr && (li & 3) == 0;
+        unsigned long long me = 0ull, seen = ~0ull;
+        const unsigned long long* pp = tp.progress + (blockIdx.x ^ (unsigned)(lane & 3));
+        if (paced) {
+          me = tp.epoch | ((unsigned long long)(unsigned)(work / (int)gridDim.x) << 16) | (unsigned long long)min(cur.m, 0xffffu);
+          if (lane == 0) asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(tp.progress + blockIdx.x), "l"(me) : "memory");
+          if (lane >= 1 && lane <= 3) asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(seen) : "l"(pp) : "memory");
+        }
         for (int q0 = 0; q0 < P.Q; q0 += (int)qs) {
           const bool mine = lane >= q0 && lane < q0 + (int)qs;
           const unsigned total = __reduce_add_sync(0xffffffffu, mine ? cur.bytes : 0u);
           const bool last_stage = li >= last_li && q0 + (int)qs >= P.Q;
           TC_PROF_WAIT(1, if (lane == 0) mbar_wait_park(b_empty0 + 8 * s, ph ^ 1u); __syncwarp())
           __syncwarp();
+          if (paced && q0 == 0) {
+            if (lane >= 1 && lane <= 3)
+              for (int spin = 0; seen + (unsigned long long)tp.pace < me && spin < 4000; ++spin) {
+                __nanosleep(64);
+                asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(seen) : "l"(pp) : "memory");
+              }
+            __syncwarp();
+          }
           if (mine) {
             const unsigned slot_u16 = (stage0 + (s * qs + (unsigned)(lane - q0)) * stage_bytes) >> 4;   // the item's window slot
 #pragma unroll
@@ -341,6 +366,11 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
           if (++s == (unsigned)tp.n_stages) { s = 0; ph ^= 1u; }
           __syncwarp();
         }
+      }
+      // this tile's list is through: the partners need not wait for this CTA before its next tile
+      if (tp.progress && lane == 0) {
+        const unsigned long long me = tp.epoch | ((unsigned long long)(unsigned)(work / (int)gridDim.x) << 16) | 0xffffull;
+        asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(tp.progress + blockIdx.x), "l"(me) : "memory");
       }
     }
     TC_PROF_END

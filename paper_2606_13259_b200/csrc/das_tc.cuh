@@ -107,6 +107,9 @@ struct TcDev {
   double z_array, kappa, ratio, phase0;
   float four_f2, kappa_f, ratio_f;
   unsigned long long* prof;    // cycle accounting per (CTA, warp), only in -DDAS_TC_PROF builds (else nullptr)
+  unsigned long long* progress;// [grid] quad pacing of the TMA producers (das_tc.cu), nullptr = off
+  unsigned long long epoch;    // launch counter << 40: progress words of earlier launches compare as far behind
+  int pace;                    // receivers a producer may run ahead of the slowest CTA of its quad
 };
 
 constexpr float kTcDelta = 1.0f / 128;      // samples: the window kernel widens every delay by this much, so that

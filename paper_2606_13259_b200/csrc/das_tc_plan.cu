@@ -1,6 +1,7 @@
 // Host side of the frame-batch tensor-core kernel (das_tc.cuh): applicability, voxel tiles,
 // per-tile receiver lists with per-group delay bounds, stage sizing, batch-inner convert kernel.
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -17,6 +18,7 @@ namespace das {
 cudaError_t launch_tc_kernel(const TcDev& tp, const Params& P, const void* tmap, void* d_out, int grid, size_t smem, cudaStream_t s);
 
 struct TcPlan {
+  mutable std::atomic<unsigned long long> launches{0};   // epoch of the quad pacing words
   TcDev dev{};
   int grid = 1;
   size_t smem = 0;
@@ -212,26 +214,48 @@ static TcPlan* tc_plan_create_groups(const Params& P, const das_plan_desc_t& d, 
   }
   if (stats[1] & 4) return refuse_free("internal: window start out of range");
 
-  // Tile order: depth slab by depth slab (heaviest slab first), all lateral tiles of a slab side by
-  // side.  The CTAs of a wave then walk the same receivers of the same depth at about the same
-  // time, so the sample windows one CTA pulls from HBM are found in L2 by its lateral neighbours
-  // (they overlap almost entirely); the cheap shallow slabs come last and level the tail.
+  // Tile order: depth slab by depth slab (heaviest slab first), inside a slab 2 x 2 blocks of laterally adjacent
+  // tiles ("quads", heaviest first), the four tiles of a quad side by side in the list.  The grid is a multiple of
+  // four CTAs and CTA c takes the list entries c, c + grid, ..., so CTAs 4 j .. 4 j + 3 always hold one quad: their
+  // receiver lists and sample windows overlap almost entirely, and the kernel's producers pace each other (das_tc.cu,
+  // "quad pacing") so that the windows one CTA pulls from HBM are found in L2 by the other three.  A quad at the
+  // rim of an odd tile grid is filled up with empty tiles.
   std::vector<double> slab_work(ntz, 0.0);
   for (int i = 0; i < n_tiles; ++i) slab_work[i / (ntx * nty)] += work[i];
-  std::vector<int> order(n_tiles);
-  std::iota(order.begin(), order.end(), 0);
-  std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
-    const int sa = a / (ntx * nty), sb = b / (ntx * nty);
-    if (sa != sb) return slab_work[sa] > slab_work[sb];
-    return work[a] > work[b];
+  const int nqx = (ntx + 1) / 2, nqy = (nty + 1) / 2;
+  struct Quad { int tz; int t[4]; double w; };
+  std::vector<Quad> quads;
+  quads.reserve((size_t)ntz * nqx * nqy);
+  for (int tz = 0; tz < ntz; ++tz)
+    for (int qy = 0; qy < nqy; ++qy)
+      for (int qx = 0; qx < nqx; ++qx) {
+        Quad qd{tz, {-1, -1, -1, -1}, 0.0};
+        for (int mth = 0; mth < 4; ++mth) {
+          const int txi = 2 * qx + (mth & 1), ty = 2 * qy + (mth >> 1);
+          if (txi < ntx && ty < nty) { qd.t[mth] = (tz * nty + ty) * ntx + txi; qd.w += work[qd.t[mth]]; }
+        }
+        quads.push_back(qd);
+      }
+  std::stable_sort(quads.begin(), quads.end(), [&](const Quad& a, const Quad& b) {
+    if (a.tz != b.tz) return slab_work[a.tz] > slab_work[b.tz];
+    return a.w > b.w;
   });
-  std::vector<TcTile> tiles_s(n_tiles);
-  std::vector<int> tbase_s(tbase.size());
-  for (int i = 0; i < n_tiles; ++i) {
-    tiles_s[i] = tiles[order[i]];
-    tiles_s[i].edge = edge[order[i]];
-    std::memcpy(&tbase_s[(size_t)i * Q], &tbase[(size_t)order[i] * Q], sizeof(int) * Q);
-  }
+  const int n_tiles_q = 4 * (int)quads.size();
+  std::vector<TcTile> tiles_s(n_tiles_q);
+  std::vector<int> tbase_s((size_t)n_tiles_q * Q, 0);
+  for (size_t u = 0; u < quads.size(); ++u)
+    for (int mth = 0; mth < 4; ++mth) {
+      const size_t i = 4 * u + mth;
+      const int t0 = quads[u].t[mth];
+      if (t0 >= 0) {
+        tiles_s[i] = tiles[t0];
+        tiles_s[i].edge = edge[t0];
+        std::memcpy(&tbase_s[i * Q], &tbase[(size_t)t0 * Q], sizeof(int) * Q);
+      } else {
+        tiles_s[i] = TcTile{d.nx, d.ny, d.nz, 0, 0, 0};        // no voxel, no receiver
+      }
+    }
+  dv.n_tiles = n_tiles_q;
   if ((e = up(tp, tiles_s, &dv.tiles)) != cudaSuccess || (e = up(tp, tbase_s, &dv.tbase)) != cudaSuccess) return fail(e);
 
   static_assert(kTcG * 2 * 64 + kTcG * kTcABufs * kTcACols <= kTcTmemCols, "accumulators + A slots exceed tensor memory");
@@ -247,7 +271,19 @@ static TcPlan* tc_plan_create_groups(const Params& P, const das_plan_desc_t& d, 
   while (dv.n_stages > kTcMinStages && tc_smem_bytes(Bc, dv.qs, dv.n_stages) > 200 * 1024) --dv.n_stages;
   tp->smem = tc_smem_bytes(Bc, dv.qs, dv.n_stages);
   if (tp->smem > 200 * 1024) return refuse_free("stage ring does not fit in shared memory");
-  tp->grid = std::max(1, std::min(n_tiles * dv.n_chunks, prop.multiProcessorCount));
+  tp->grid = std::max(4, std::min(dv.n_tiles * dv.n_chunks, prop.multiProcessorCount) / 4 * 4);
+  // quad pacing: one progress word per CTA (DAS_TC_PACE = 0 switches it off, any other value sets the lead in receivers)
+  dv.pace = 16;
+  if (const char* ev = getenv("DAS_TC_PACE")) dv.pace = atoi(ev);                                                        // tuning sweeps only
+  dv.progress = nullptr;
+  dv.epoch = 0;
+  if (dv.pace > 0) {
+    void* dp = nullptr;
+    if ((e = cudaMalloc(&dp, sizeof(unsigned long long) * tp->grid)) != cudaSuccess) return fail(e);
+    tp->allocs.push_back(dp);
+    if ((e = cudaMemset(dp, 0, sizeof(unsigned long long) * tp->grid)) != cudaSuccess) return fail(e);
+    dv.progress = static_cast<unsigned long long*>(dp);
+  }
   return tp;
 }
 
@@ -310,7 +346,9 @@ cudaError_t launch_tc(const TcPlan* tp, const Params& P, const void* d_conv, voi
     return e;
   }
 #endif
-  return launch_tc_kernel(tp->dev, P, map, d_out, tp->grid, tp->smem, s);
+  TcDev dv = tp->dev;
+  dv.epoch = (tp->launches.fetch_add(1) + 1) << 40;       // concurrent launches of one plan only blur the pacing (it is advisory)
+  return launch_tc_kernel(dv, P, map, d_out, tp->grid, tp->smem, s);
 }
 
 // ---- batch-inner layout transform + cast (PAPER.md:149 permute to batch-inner, :194-200 FP16) ----
