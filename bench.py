@@ -448,7 +448,7 @@ def run_cuda(args):
     h_outs = [torch.empty(tuple(out.shape), dtype=out.dtype).pin_memory() for _ in range(2)]
     h_out = h_outs[0]
     plan.beamform_host(h_raw[0].data_ptr(), h_out.data_ptr(), sp)          # allocates the staging
-    e_steps = max(2, args.e2e_steps if B == 1 else min(args.e2e_steps, 4))
+    e_steps = max(2, args.e2e_steps if B == 1 else min(args.e2e_steps, 8))    # 8 x 8.6 GB over PCIe: 1.3 s
     e_beg, e_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     t_wall = time.perf_counter()
@@ -552,6 +552,7 @@ def run_cuda(args):
         # wavefronts); the FP32-ALU figures stay beside it as `alu_roofline`
         sf["alu_roofline"] = {k: sf[k] for k in ("achieved", "peak", "unit", "frac")}
         sf["bound"] = name
+        sf["achieved"], sf["peak"], sf["unit"] = pct, 100.0, "% of the pipe's peak (ncu)"
         sf["frac"] = pct / 100.0
         sf["frac_how"] = "ncu utilisation of the binding pipe in the committed capture (not re-measured in this run)"
     # both readings of the metric at top level: B frames per call (value) and one frame per call

@@ -327,7 +327,7 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
         // Advisory only: the wait is bounded, nothing else depends on it.
         // The partners' words are loaded here and looked at only after the wait for the stage below, so that the
         // round trip to L2 hides under it; one receiver in four is paced.
-        const bool paced = tp.progress != nullptr && (li & 3) == 0;
+        const bool paced = tp.progress != nullptr && (li & tp.pace_mask) == 0;
         unsigned long long me = 0ull, seen = ~0ull;
         const unsigned long long* pp = tp.progress + (blockIdx.x ^ (unsigned)(lane & 3));
         if (paced) {

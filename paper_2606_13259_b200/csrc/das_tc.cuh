@@ -110,6 +110,7 @@ struct TcDev {
   unsigned long long* progress;// [grid] quad pacing of the TMA producers (das_tc.cu), nullptr = off
   unsigned long long epoch;    // launch counter << 40: progress words of earlier launches compare as far behind
   int pace;                    // receivers a producer may run ahead of the slowest CTA of its quad
+  int pace_mask;               // a receiver is paced when (list index & pace_mask) == 0
 };
 
 constexpr float kTcDelta = 1.0f / 128;      // samples: the window kernel widens every delay by this much, so that

@@ -275,6 +275,8 @@ static TcPlan* tc_plan_create_groups(const Params& P, const das_plan_desc_t& d, 
   // quad pacing: one progress word per CTA (DAS_TC_PACE = 0 switches it off, any other value sets the lead in receivers)
   dv.pace = 16;
   if (const char* ev = getenv("DAS_TC_PACE")) dv.pace = atoi(ev);                                                        // tuning sweeps only
+  dv.pace_mask = 3;
+  if (const char* ev = getenv("DAS_TC_PACE_MASK")) dv.pace_mask = atoi(ev);                                             // tuning sweeps only
   dv.progress = nullptr;
   dv.epoch = 0;
   if (dv.pace > 0) {
