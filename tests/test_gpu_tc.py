@@ -257,3 +257,26 @@ def test_tc_beamform_host_pipelined(das_lib):
     plan.beamform_host_wait()
     np.testing.assert_array_equal(h_out[2].numpy(), want[2])
     plan.destroy()
+
+
+@pytest.mark.timeout(180)
+def test_tc_repeated_launches_deterministic(das_lib):
+    """Soak: the warp roles of tc_kernel hand data over through five mbarrier rings, tensor memory and (quad pacing)
+    global progress words.  500 launches back to back on config 2 with 16 frames must neither hang nor change a bit
+    (a voxel's terms are accumulated in a fixed order, so the kernel is deterministic)."""
+    torch = _torch()
+    das = das_lib
+    w = wl.config(2, generate_data=False)
+    plan = das.Plan.from_workload(w, storage=das.STORE_FP16, algo=das.ALGO_TC, n_frames=16)
+    g = torch.Generator(device="cuda").manual_seed(5)
+    raw = torch.view_as_complex(torch.randn((16, w.n_tx, w.n_elem, w.n_samples, 2), device="cuda", generator=g) * 0.1)
+    conv = torch.empty(plan.converted_bytes, dtype=torch.uint8, device="cuda")
+    outs = [torch.empty(plan.output_bytes // 4, dtype=torch.float32, device="cuda") for _ in range(2)]
+    s = torch.cuda.current_stream().cuda_stream
+    plan.convert(raw.data_ptr(), conv.data_ptr(), 1.0, s)
+    plan.execute(conv.data_ptr(), outs[0].data_ptr(), s)
+    for _ in range(500):
+        plan.execute(conv.data_ptr(), outs[1].data_ptr(), s)
+    torch.cuda.synchronize()
+    assert torch.equal(outs[0], outs[1])
+    plan.destroy()
