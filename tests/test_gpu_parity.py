@@ -414,3 +414,72 @@ def test_tiled_kernel_repeated_launches_do_not_hang(das_lib, monkeypatch):
     torch.cuda.synchronize()
     assert torch.equal(outs[0], outs[1])
     plan.destroy()
+
+
+@pytest.mark.parametrize("n_tx", [17, 33])
+@pytest.mark.parametrize("kind", [wl.DATA_IQ, wl.DATA_RF])
+@pytest.mark.parametrize("storage", [0, 1])
+def test_more_than_16_transmits_chunked(das_lib, n_tx, kind, storage):
+    """More than 16 transmits: the tiled kernel walks the receivers once per chunk of 16 transmits (n_chunks > 1:
+    the producer / converter stage counters and the per-chunk phase table are reused), which no BASELINE config
+    exercises (ADVICE, round 1).  Mixed plane / diverging transmits, 6 x 6 array, ragged 19 x 13 x 21 grid."""
+    import oracle
+    das = das_lib
+    rng = np.random.default_rng(100 + n_tx)
+    elem = wl.matrix_array(6)
+    tx_type, tx_v, tx_t0 = [], [], []
+    for q in range(n_tx):
+        if q % 3 == 2:
+            tx_type.append(wl.TX_DIVERGING)
+            tx_v.append([rng.uniform(-1e-3, 1e-3), rng.uniform(-1e-3, 1e-3), -rng.uniform(4e-3, 8e-3)])
+            tx_t0.append(-float(np.linalg.norm(tx_v[-1])) / wl.C0)
+        else:
+            a, b = np.radians(rng.uniform(-8, 8, 2))
+            tx_type.append(wl.TX_PLANE)
+            tx_v.append([np.sin(a), np.sin(b), np.sqrt(1 - np.sin(a) ** 2 - np.sin(b) ** 2)])
+            tx_t0.append(rng.uniform(0, 2e-7))
+    xs, ys, zs = wl.axis(-1.2e-3, 1.1e-3, 19), wl.axis(-0.9e-3, 1.0e-3, 13), wl.axis(1.5e-3, 6e-3, 21)
+    pos = np.stack([rng.uniform(-1e-3, 1e-3, 5), rng.uniform(-0.8e-3, 0.8e-3, 5), rng.uniform(2e-3, 5.5e-3, 5)], 1)
+    fs = 15.6e6 if kind == wl.DATA_IQ else 31.2e6
+    w = wl.custom(elem, tx_type, tx_v, tx_t0, xs, ys, zs, fs=fs, n_samples=320 if kind == wl.DATA_IQ else 640,
+                  data_kind=kind, scat_pos=pos, scat_amp=rng.uniform(0.3, 1, 5), noise_sigma=0.01, seed=9)
+    ref = oracle.das(w)
+    for algo in (das.ALGO_TILED, das.ALGO_GENERAL):
+        out, used = gpu_das(das, w, storage, algo)
+        assert used == algo
+        check(out, ref, storage, das, f"{n_tx} transmits, algo {algo}")
+
+
+@pytest.mark.parametrize("algo_name", ["tiled", "general"])
+def test_record_edges_with_large_samples(das_lib, algo_name):
+    """Reading A6 at the ends of the record with LARGE samples at k = 0, 1, K-2, K-1 (ADVICE, round 1: the edge rule is
+    a step, and an index misrounded there would add or drop a whole |y_0| or |y_K-1| term; noise-level edge samples
+    would hide it).  The grid is placed so that many (q, m, n) terms have floor(t) in {-1, 0} and {K-2, K-1}; the
+    term counts must equal the oracle's exactly and the fp32 result must meet the fp32 gate."""
+    import oracle
+    das = das_lib
+    algo = das.ALGO_TILED if algo_name == "tiled" else das.ALGO_GENERAL
+    rng = np.random.default_rng(77)
+    elem = wl.matrix_array(6)
+    K, fs = 96, 15.6e6
+    # two-way travel time to depth z is about 2 z / c: t = 0 near z = t_start c / 2, t = K - 1 near (t_start + (K-1)/fs) c / 2
+    t_start = 3.0e-6
+    z0, z1 = t_start * wl.C0 / 2, (t_start + (K - 1) / fs) * wl.C0 / 2
+    zs = np.concatenate([np.linspace(z0 - 60e-6, z0 + 120e-6, 12), np.linspace(z1 - 120e-6, z1 + 60e-6, 12)])   # 3 + 3 depth tiles
+    xs, ys = wl.axis(-0.6e-3, 0.6e-3, 9), wl.axis(-0.5e-3, 0.5e-3, 8)
+    y = (rng.normal(size=(2, 36, K)) + 1j * rng.normal(size=(2, 36, K))).astype(np.complex64) * np.float32(0.01)
+    for k in (0, 1, K - 2, K - 1):
+        y[:, :, k] = (rng.uniform(5, 10, (2, 36)) * np.exp(2j * np.pi * rng.uniform(size=(2, 36)))).astype(np.complex64)
+    w = wl.custom(elem, [wl.TX_PLANE, wl.TX_PLANE], [[0, 0, 1], [np.sin(0.05), 0, np.cos(0.05)]], [0.0, 1e-8], xs, ys, zs,
+                  fs=fs, n_samples=K, t_start=t_start, f_number=0.0, y=y)
+    res = oracle.das(w, want_count=True)
+    ref, cnt = res["out"], res["count"]
+    out, used = gpu_das(das, w, das.STORE_FP32, algo)
+    assert used == algo
+    k_edge = int((cnt < w.n_elem * w.n_tx).sum())
+    assert k_edge > 50, "the case must have voxels that lose terms at the record ends"
+    check(out, ref, das.STORE_FP32, das, "record edges")
+    plan = das.Plan.from_workload(w, storage=das.STORE_FP32, algo=algo)
+    pairs, terms = plan.count_work()
+    plan.destroy()
+    assert terms == int(cnt.sum())
