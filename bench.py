@@ -514,8 +514,10 @@ def run_cuda(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
         "warmup": args.warmup, "ms_per_step": total_ms / steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32" if B == 1 else "f16 x f16 -> f32", "data": "synthetic",
-        "config": {"workload": workload_name(w, args.storage) + (f"; {B} frames per call (configs[4] ensemble)" if B > 1 else ""),
+        "config": {"workload": workload_name(w, args.storage),     # the same string in both arms; B is its own key
                    "kernel": algo_used, "frames_per_call": B,
+                   "frames": (f"{B} frames per call (configs[4] ensemble), one das_convert + one das_execute per {B} frames"
+                              if B > 1 else "one frame per call"),
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"{raw_bytes / 1e6:.0f} MB of distinct raw input per rotation + {convbytes / 1e6:.0f} MB converted "
                          f"buffer rewritten every step > 126 MB L2",
