@@ -151,7 +151,11 @@ das_status_t das_convert(const das_plan_t* plan, const void* d_raw, void* d_conv
  *           them (DAS_ALGO_TC: batch-inner [chunk][M][Q][column group][2K][8] FP16; else [M][Q][Kp] intervals);
  *           a buffer converted for another layout is not detected
  *   d_out   device, das_output_bytes() bytes, [B][nx][ny][nz] with z fastest (C order), complex64
- *           (IQ) or float32 (RF); overwritten, not accumulated into; 8-byte aligned */
+ *           (IQ) or float32 (RF); overwritten, not accumulated into; 8-byte aligned
+ * Calls on one plan may overlap (different streams, different buffers).  For DAS_ALGO_TC the CTAs of a launch pace
+ * each other through progress words owned by the plan (L2 reuse between neighbouring tiles): overlapping launches
+ * of ONE such plan stay correct (the pacing is advisory and its waits are bounded) but lose the pacing's benefit;
+ * use one plan per stream. */
 das_status_t das_execute(const das_plan_t* plan, const void* d_conv, void* d_out, void* stream);
 
 /* End-to-end convenience for HOST buffers: copies h_raw to the device, runs das_convert
