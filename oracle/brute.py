@@ -103,11 +103,24 @@ def das(w, y=None, **opts) -> np.ndarray:
     return x if int(w.data_kind) == 0 else x.real
 
 
-def das_from_interval_table(w, mid, slope) -> np.ndarray:
+def das_from_interval_table(w, mid, slope, **unsupported) -> np.ndarray:
     """The definition evaluated on a given table of sample INTERVALS: y[t] = mid_k + (alpha - 1/2) slope_k for
     t = k + alpha (equal to linear interpolation, when mid_k = (y_k + y_k+1)/2 and
     slope_k = y_k+1 - y_k).  ``mid`` / ``slope``: [Q, M, K-1].  Used to check a storage format that quantises
-    the interval table (fp8 storage) term by term instead of only statistically."""
+    the interval table (fp8 storage) term by term instead of only statistically.
+
+    Pinned by tests/test_oracle_ext_pins.py (test_interval_table_*): equal to oracle.das on the exact table of
+    random data (IQ with and without the f-number cone, RF) and the hand value of closed_form_cases.json
+    plane_345.  Boxcar aperture about (0, 0, 1) normals and the delay models of tx[] only: element normals,
+    windows, tables, lists or cubic interpolation raise instead of being ignored."""
+    if unsupported:
+        raise TypeError(f"das_from_interval_table does not take {sorted(unsupported)}")
+    if getattr(w, "elem_dir", None) is not None:
+        raise ValueError("das_from_interval_table handles (0, 0, 1) element normals only")
+    mid, slope = np.asarray(mid), np.asarray(slope)
+    want = (len(w.tx_type), len(w.elem_pos), int(w.n_samples) - 1)
+    if mid.shape != want or slope.shape != want:
+        raise ValueError(f"mid / slope must be [Q, M, K-1] = {want}, got {mid.shape} / {slope.shape}")
     e = np.asarray(w.elem_pos, dtype=np.float64)
     gx, gy, gz = np.meshgrid(np.asarray(w.xs, np.float64), np.asarray(w.ys, np.float64),
                              np.asarray(w.zs, np.float64), indexing="ij")

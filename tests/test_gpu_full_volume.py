@@ -10,7 +10,7 @@ of the seeded input; a stale or foreign cache is recomputed, never trusted.
 
 Per-voxel FP16 bound (pin P12, tests/test_oracle_pins.py): rounding the stored samples to FP16 changes a voxel
 by at most 2^-11 * l1_n, l1_n = sum over entered terms of w ((1-a)|y_k|_1 + a|y_k+1|_1).  The kernels do not
-store plain samples, so the constant differs and DESIGN.md 4.3 derives it:
+store plain samples, so the constant differs and DESIGN.md 4.3 (item 5) derives it:
   tiled kernel : stores (mid, slope) = ((y_k + y_k+1)/2, y_k+1 - y_k), each rounded: the error of one term is at
                  most 2^-11 (|y_k|_1 + |y_k+1|_1), whose sum over many terms with uniformly spread a is 2 * l1_n;
   batch kernel : stores plain FP16 samples and FP16 weights: at most (2^-11 + 2^-11 + 2^-22) per term = 2 * l1_n.

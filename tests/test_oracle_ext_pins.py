@@ -242,3 +242,69 @@ def test_slack_output_counts_near_edge_terms(oracle):
     assert abs(r["slack"][0, 0, 0] - 5.0) < 1e-12
     w2 = _one_voxel(case, u, y=y, f_number=1.0, fc=0.0, voxel=[1, 0, 4])      # well inside
     assert oracle.das(w2, want_slack=True)["slack"][0, 0, 0] == 0.0
+
+
+# ---------------------------------------------------------------- the interval-table evaluator (FP8 check helper)
+
+def _exact_table(y):
+    """(mid, slope) of PAPER.md:50's two-sample lerp, formed in FP64 from the float32 samples."""
+    yd = np.asarray(y).astype(np.complex128)
+    return 0.5 * (yd[:, :, :-1] + yd[:, :, 1:]), yd[:, :, 1:] - yd[:, :, :-1]
+
+
+@pytest.mark.parametrize("kind,f_number", [(wl.DATA_IQ, 1.0), (wl.DATA_IQ, 0.0), (wl.DATA_RF, 1.0)])
+def test_interval_table_equals_the_oracle_on_the_exact_table(oracle, kind, f_number):
+    """mid_k + (alpha - 1/2) slope_k with mid = (y_k + y_k+1)/2, slope = y_k+1 - y_k IS (1 - alpha) y_k + alpha y_k+1
+    (PAPER.md:50), so on the unquantised table oracle/brute.py::das_from_interval_table must reproduce the pinned C
+    oracle: a wrong aperture rule, a transposed mid[q][m, k], a dropped 1/2 or a wrong sign in it fails here."""
+    import oracle.brute as brute
+    w = _small_problem(21, kind=kind, f_number=f_number, n=(5, 4, 6), k=96)
+    ref = oracle.das(w)
+    mid, slope = _exact_table(w.y)
+    got = brute.das_from_interval_table(w, mid, slope)
+    assert got.shape == ref.shape and np.iscomplexobj(got) == (kind == wl.DATA_IQ)
+    assert np.abs(ref).max() > 0
+    if f_number > 0:                                  # the cone really cuts pairs in this geometry
+        assert oracle.das(w, want_count=True)["count"].sum() < oracle.das(
+            _small_problem(21, kind=kind, f_number=0.0, n=(5, 4, 6), k=96), want_count=True)["count"].sum()
+    np.testing.assert_allclose(got, ref, rtol=0, atol=1e-12 * np.abs(ref).max())
+    # a table that is NOT the lerp's must change the answer (the check above is not vacuous)
+    off = brute.das_from_interval_table(w, mid, -slope)
+    assert np.abs(off - ref).max() > 1e-3 * np.abs(ref).max()
+
+
+def test_interval_table_hand_value():
+    """closed_form_cases.json plane_345 (PAPER.md:35-37 Eq. 1, :77 fn. 2, :50): the ramp y_k = a + b k has
+    mid_k = a + b (k + 1/2), slope_k = b; t = 115.2, 0.8 turn: x = -7.3799 - 64.0136j (derived by hand there)."""
+    import oracle.brute as brute
+    with open(os.path.join(os.path.dirname(__file__), "golden", "closed_form_cases.json")) as f:
+        g = json.load(f)
+    u, case = g["u"], g["cases"][0]
+    assert case["name"] == "plane_345"
+    a, b = complex(*case["ramp_a"]), complex(*case["ramp_b"])
+    k = case["K"]
+    elem, vox = np.array(case["elem_pos_u"], np.float64) * u, np.array(case["voxel_u"], np.float64) * u
+    w = wl.custom(elem, [wl.TX_PLANE], [case["tx"]["v"]], [case["tx"]["t0"]], [vox[0]], [vox[1]], [vox[2]],
+                  fs=case["fs"], n_samples=k, c=case["c"], fc=case["fc"], t_start=case["t_start"],
+                  f_number=case["f_number"], y=_ramp(1, 1, k, a, b))
+    kk = np.arange(k - 1, dtype=np.float64)
+    mid = (a + b * (kk + 0.5)).reshape(1, 1, -1)
+    slope = np.full((1, 1, k - 1), b)
+    got = brute.das_from_interval_table(w, mid, slope)[0, 0, 0]
+    exp = complex(*case["expected"])
+    assert abs(got - exp) <= 1e-9 * abs(exp), (got, exp)
+
+
+def test_interval_table_refuses_what_it_does_not_model():
+    import oracle.brute as brute
+    w = _small_problem(5, n=(2, 2, 2), k=32)
+    mid, slope = _exact_table(w.y)
+    with pytest.raises(TypeError):
+        brute.das_from_interval_table(w, mid, slope, window="hann")
+    with pytest.raises(TypeError):
+        brute.das_from_interval_table(w, mid, slope, tau_tx=np.zeros((2, 8), np.float32))
+    with pytest.raises(ValueError):
+        brute.das_from_interval_table(w, mid[:, :, :-1], slope[:, :, :-1])
+    w.elem_dir = np.tile(np.array([0.0, 0.0, 1.0], np.float32), (len(w.elem_pos), 1))
+    with pytest.raises(ValueError):
+        brute.das_from_interval_table(w, mid, slope)
