@@ -178,6 +178,32 @@ das_status_t das_beamform_host(das_plan_t* plan, const void* h_raw, void* h_out,
 das_status_t das_beamform_host_begin(das_plan_t* plan, const void* h_raw, void* h_out, void* stream);
 das_status_t das_beamform_host_wait(das_plan_t* plan);
 
+/* The same raw -> volume path for callers that cannot allocate device memory, and for which the library must
+ * not allocate either: a real-time acquisition / display loop (cudaMalloc and cudaFree take a driver lock and may
+ * synchronise the device: a dropped frame), a plug-in inside an application whose own memory pool already owns
+ * the whole GPU (cudaMalloc just fails there), software under a "no allocation after set-up" rule.
+ * das_convert + das_execute need a converted buffer from the caller; das_beamform_host allocates staging buffers
+ * on first use.  This call needs neither: the converted data goes through a scratch array that is part of the
+ * library image (a file-scope __device__ array of DAS_STATIC_SCRATCH_BYTES, resident on every GPU that loads the
+ * library, from module load until the process exits).  It calls no cudaMalloc / cudaFree and no allocating
+ * library routine, synchronises nothing, and enqueues exactly the kernels of das_convert(scale) + das_execute on
+ * `stream`, so the result is bit-identical to theirs.
+ *   d_raw, d_out   device, as for das_convert / das_execute (inputs and outputs stay the caller's)
+ *   limit          das_converted_bytes(plan) <= DAS_STATIC_SCRATCH_BYTES, else DAS_ERR_SIZE and nothing is
+ *                  enqueued (16 MiB takes BASELINE.json configs 1 and 2; the headline needs 151 MB: use
+ *                  das_convert + das_execute with your own buffer there)
+ *   first call     the first call on each device looks the array's device address up (cudaGetSymbolAddress,
+ *                  which loads the CUDA module on that device if it is not loaded yet).  Make that call during
+ *                  set-up, before any stream capture and before the no-allocation phase begins.
+ *   sharing        there is ONE array per GPU for the whole process: two das_beamform_static calls that can
+ *                  overlap on the GPU (different streams, or different plans on different streams) race on it
+ *                  and give garbage.  Keep all calls of one GPU on one stream, or order them with events.  The
+ *                  array keeps the last call's bytes between calls; nothing in it has to be cleared, because
+ *                  das_convert rewrites every byte das_execute reads. */
+#define DAS_STATIC_SCRATCH_BYTES (16u << 20)
+das_status_t das_beamform_static(const das_plan_t* plan, const void* d_raw, void* d_out, float scale,
+                                 void* stream);
+
 /* Work accounting (used by the bench's roofline; not part of the hot path).  Runs a counting
  * kernel on the plan's device and SYNCHRONISES.  On success
  *   *n_pairs = number of (m, n) receiver/voxel pairs with non-zero receive weight w_rx

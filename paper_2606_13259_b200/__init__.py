@@ -29,11 +29,12 @@ STORE_FP32, STORE_FP16, STORE_FP8 = 0, 1, 2
 ALGO_AUTO, ALGO_GENERAL, ALGO_TILED, ALGO_TC = 0, 1, 2, 3
 WINDOW_BOXCAR, WINDOW_HANN, WINDOW_TUKEY = 0, 1, 2
 INTERP_LINEAR, INTERP_CUBIC = 0, 1
+STATIC_SCRATCH_BYTES = 16 << 20        # DAS_STATIC_SCRATCH_BYTES of include/das.h
 
 # every symbol include/das.h declares (checked against the header by tests/test_abi.py)
 EXPORTS = ("das_plan_create", "das_plan_destroy", "das_raw_bytes", "das_converted_bytes",
            "das_output_bytes", "das_plan_algo", "das_plan_frames", "das_convert", "das_execute", "das_beamform_host",
-           "das_beamform_host_begin", "das_beamform_host_wait",
+           "das_beamform_host_begin", "das_beamform_host_wait", "das_beamform_static",
            "das_plan_count_work", "das_status_string", "das_last_error", "das_launch_count")
 
 
@@ -107,6 +108,8 @@ def load(build_if_missing: bool = True):
     lib.das_beamform_host_begin.argtypes = [vp, vp, vp, vp]
     lib.das_beamform_host_wait.restype = ctypes.c_int
     lib.das_beamform_host_wait.argtypes = [vp]
+    lib.das_beamform_static.restype = ctypes.c_int
+    lib.das_beamform_static.argtypes = [vp, vp, vp, ctypes.c_float, vp]
     lib.das_plan_count_work.restype = ctypes.c_int
     lib.das_plan_count_work.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong), ctypes.POINTER(ctypes.c_ulonglong)]
     lib.das_status_string.restype = ctypes.c_char_p
@@ -249,6 +252,12 @@ class Plan:
 
     def beamform_host_wait(self):
         _check(self._lib.das_beamform_host_wait(self._h))
+
+    def beamform_static(self, d_raw: int, d_out: int, scale: float = 1.0, stream: int = 0):
+        """das_beamform_static: das_convert + das_execute through the library's built-in 16 MiB scratch array,
+        for callers that cannot allocate device memory (include/das.h).  Device pointers in, nothing allocated."""
+        _check(self._lib.das_beamform_static(self._h, ctypes.c_void_p(d_raw), ctypes.c_void_p(d_out),
+                                             ctypes.c_float(scale), ctypes.c_void_p(stream)))
 
     def count_work(self):
         """(n_pairs, n_terms) of das_plan_count_work: active (m, n) pairs and entered (q, m, n) terms."""

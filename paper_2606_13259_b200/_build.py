@@ -14,7 +14,7 @@ LIB = os.path.join(HERE, "libdas_b200.so")
 OBJ_DIR = os.path.join(HERE, "build")
 
 SOURCES = ["das_api.cu", "das_convert.cu", "das_general.cu", "das_tiled_plan.cu",
-           "das_tc.cu", "das_tc_plan.cu",
+           "das_tc.cu", "das_tc_plan.cu", "das_static.cu",
            "das_tiled_inst_iq32.cu", "das_tiled_inst_iq16.cu", "das_tiled_inst_rf32.cu", "das_tiled_inst_rf16.cu",
            "das_tiled_inst_iq8.cu", "das_tiled_inst_rf8.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -468,3 +468,9 @@ das_status_t das_plan_count_work(const das_plan_t* p, unsigned long long* n_pair
 
 #pragma GCC visibility pop
 }  // extern "C"
+
+// What das_static.cu (das_beamform_static) needs from the opaque plan and the error channel.
+namespace das {
+int plan_device(const das_plan* p) { return p->device; }
+void set_error_text(const char* msg) { set_err("%s", msg); }
+}  // namespace das

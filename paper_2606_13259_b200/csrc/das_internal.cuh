@@ -114,4 +114,8 @@ cudaError_t launch_tiled(const TiledPlan* tp, const Params& P, const void* d_con
 
 void count_launch(unsigned long long n = 1);
 
+// das_api.cu, for das_static.cu: the plan's device ordinal and the thread-local das_last_error() text
+int plan_device(const das_plan* p);
+void set_error_text(const char* msg);
+
 }  // namespace das
