@@ -259,6 +259,11 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
     // full barrier.  Bit 31 of a stage's first info word marks the last stage of a tile.
     unsigned s = 0, ph = 0;                                  // stage and its phase parity
     const bool has_q = lane < P.Q;
+    // quad pacing (below): what lanes 1..3 may still spend waiting for their partner CTA.  A wait that runs its
+    // budget out quarters it, so a partner that is not there (not co-resident: an SM limit, a kernel of another
+    // stream on its SM; or simply far behind) costs this CTA about 5 300 polls per LAUNCH (a few ms), not 4 000
+    // per paced receiver, and after six expiries the lane stops looking at that partner.
+    int pace_budget = 4000;
     TC_PROF_DECL
     for (int work = blockIdx.x; work < n_work; work += gridDim.x) {
       const int tile_i = work % tp.n_tiles, chunk = work / tp.n_tiles;
@@ -324,7 +329,7 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
         // receiver lists and sample windows overlap almost entirely.  Each producer publishes (launch, round, receiver)
         // before it fetches a receiver's windows and holds back while a partner is more than `pace` receivers behind:
         // the four then read the same records within microseconds of each other and three of the four reads hit L2.
-        // Advisory only: the wait is bounded, nothing else depends on it.
+        // Advisory only: the wait is bounded per receiver and per launch (pace_budget), nothing else depends on it.
         // The partners' words are loaded here and looked at only after the wait for the stage below, so that the
         // round trip to L2 hides under it; one receiver in four is paced.
         const bool paced = tp.progress != nullptr && (li & tp.pace_mask) == 0;
@@ -333,7 +338,7 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
         if (paced) {
           me = tp.epoch | ((unsigned long long)(unsigned)(work / (int)gridDim.x) << 16) | (unsigned long long)min(cur.m, 0xffffu);
           if (lane == 0) asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(tp.progress + blockIdx.x), "l"(me) : "memory");
-          if (lane >= 1 && lane <= 3) asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(seen) : "l"(pp) : "memory");
+          if (lane >= 1 && lane <= 3 && pace_budget > 0) asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(seen) : "l"(pp) : "memory");
         }
         for (int q0 = 0; q0 < P.Q; q0 += (int)qs) {
           const bool mine = lane >= q0 && lane < q0 + (int)qs;
@@ -342,11 +347,14 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
           TC_PROF_WAIT(1, if (lane == 0) mbar_wait_park(b_empty0 + 8 * s, ph ^ 1u); __syncwarp())
           __syncwarp();
           if (paced && q0 == 0) {
-            if (lane >= 1 && lane <= 3)
-              for (int spin = 0; seen + (unsigned long long)tp.pace < me && spin < 4000; ++spin) {
+            if (lane >= 1 && lane <= 3) {
+              int spin = 0;
+              for (; seen + (unsigned long long)tp.pace < me && spin < pace_budget; ++spin) {
                 __nanosleep(64);
                 asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(seen) : "l"(pp) : "memory");
               }
+              if (spin > 0 && spin >= pace_budget) pace_budget >>= 2;          // expired: this partner gets less from now on
+            }
             __syncwarp();
           }
           if (mine) {

@@ -300,3 +300,45 @@ def test_tc_quad_pacing_does_not_change_results(das_lib, monkeypatch):
         outs.append(out.clone())
         plan.destroy()
     assert torch.equal(torch.view_as_real(outs[0]), torch.view_as_real(outs[1]))
+
+
+def test_tc_pacing_gives_up_on_a_partner_that_is_not_resident(das_lib):
+    """ADVICE (round 2): the quad pacing must not turn a missing partner into seconds.  A one-thread spinning kernel
+    on a side stream holds one SM's registers, so one of the persistent CTAs (512 threads x 128 registers = the whole
+    register file) cannot start until another CTA has finished: its three partners see a progress word that never
+    moves.  Each paced receiver used to wait the full 4 000 polls (about 1 s in total on this problem); with the
+    shrinking budget (das_tc.cu, pace_budget) the launch costs the serialised CTA's work plus a few ms.  The
+    volume stays bit-identical, as the pacing is advisory."""
+    import time
+    torch = _torch()
+    das = das_lib
+    w = _cfg(2)                                       # 64^3 voxels: 704 tiles, one CTA on every SM
+    g = torch.Generator(device="cuda").manual_seed(5)
+    raw = torch.view_as_complex(torch.randn((8, w.n_tx, w.n_elem, w.n_samples, 2), device="cuda", generator=g) * 0.1)
+    plan = das.Plan.from_workload(w, storage=das.STORE_FP16, algo=das.ALGO_TC, n_frames=8)
+    out, conv = das.beamform_torch(plan, raw)
+    torch.cuda.synchronize()
+    ref = out.clone()
+    main = torch.cuda.current_stream()
+
+    def timed():
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        out.fill_(0)
+        e0.record(main)
+        plan.execute(conv.data_ptr(), out.data_ptr(), main.cuda_stream)
+        e1.record(main)
+        e1.synchronize()
+        return e0.elapsed_time(e1)
+
+    t_alone = min(timed() for _ in range(3))
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        torch.cuda._sleep(int(6e8))                   # about 0.3 s on one SM, far longer than the launch
+    time.sleep(0.02)                                  # let it start before the batch kernel is enqueued
+    t_hog = timed()
+    busy = not side.query()                           # the hog outlived the launch it was meant to disturb
+    side.synchronize()
+    print(f"tc_kernel alone {t_alone:.2f} ms, with one SM taken {t_hog:.2f} ms (hog still running: {busy})")
+    assert torch.equal(torch.view_as_real(out), torch.view_as_real(ref))
+    assert t_hog <= 3.0 * t_alone + 25.0, (t_alone, t_hog)
+    plan.destroy()
