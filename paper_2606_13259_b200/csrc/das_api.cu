@@ -4,6 +4,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <initializer_list>
 #include <new>
 #include <vector>
 
@@ -390,14 +391,13 @@ static das_status_t host_staging(das_plan* p) {
   for (auto& sl : p->slot) {
     if ((e = cudaMalloc(&sl.d_raw, p->raw_bytes)) != cudaSuccess || (e = cudaMalloc(&sl.d_out, p->out_bytes)) != cudaSuccess)
       return fail("allocating staging buffers");
-    if (!sl.ev_h2d && ((e = cudaEventCreateWithFlags(&sl.ev_h2d, cudaEventDisableTiming)) != cudaSuccess ||
-                       (e = cudaEventCreateWithFlags(&sl.ev_exec, cudaEventDisableTiming)) != cudaSuccess ||
-                       (e = cudaEventCreateWithFlags(&sl.ev_d2h, cudaEventDisableTiming)) != cudaSuccess))
-      return fail("creating events");
+    for (cudaEvent_t* ev : {&sl.ev_h2d, &sl.ev_exec, &sl.ev_d2h})
+      if (!*ev && (e = cudaEventCreateWithFlags(ev, cudaEventDisableTiming)) != cudaSuccess) { *ev = nullptr; return fail("creating events"); }
   }
-  if (!p->s_in && ((e = cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking)) != cudaSuccess ||
-                   (e = cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking)) != cudaSuccess))
-    return fail("creating copy streams");
+  // each stream under its own check: after a partial failure the next call must not take a missing s_out for
+  // "both exist" and copy out on the legacy default stream
+  if (!p->s_in && (e = cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking)) != cudaSuccess) { p->s_in = nullptr; return fail("creating copy streams"); }
+  if (!p->s_out && (e = cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking)) != cudaSuccess) { p->s_out = nullptr; return fail("creating copy streams"); }
   if ((e = cudaMalloc(&p->st_conv, p->conv_bytes)) != cudaSuccess) return fail("allocating staging buffers");
   return DAS_OK;
 }
@@ -412,6 +412,12 @@ das_status_t das_beamform_host_begin(das_plan_t* p, const void* h_raw, void* h_o
   das_plan::HostSlot& sl = p->slot[p->begun & 1];
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   cudaError_t e;
+  // A failure after the first enqueue leaves copies / kernels of this call in flight on a slot that is not
+  // recorded as begun: drain the three streams before reporting it, so that the next begin finds the slot idle.
+  struct Drain {
+    das_plan* p; cudaStream_t s; bool armed = true;
+    ~Drain() { if (armed) { cudaStreamSynchronize(p->s_in); cudaStreamSynchronize(s); cudaStreamSynchronize(p->s_out); } }
+  } drain{p, s};
   // slot reuse: the previous user's kernels have read d_raw (ev_exec), its copy-out has read d_out (ev_d2h)
   if (sl.used && (e = cudaStreamWaitEvent(p->s_in, sl.ev_exec, 0)) != cudaSuccess) return cuda_fail(e, "stream wait");
   if ((e = cudaMemcpyAsync(sl.d_raw, h_raw, p->raw_bytes, cudaMemcpyHostToDevice, p->s_in)) != cudaSuccess)
@@ -428,6 +434,7 @@ das_status_t das_beamform_host_begin(das_plan_t* p, const void* h_raw, void* h_o
   if ((e = cudaEventRecord(sl.ev_d2h, p->s_out)) != cudaSuccess) return cuda_fail(e, "event record");
   sl.used = true;
   ++p->begun;
+  drain.armed = false;
   return DAS_OK;
 }
 
