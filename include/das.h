@@ -25,8 +25,9 @@
  *     belong to the plan's CUDA device.  The library never takes ownership of caller memory.
  *   - das_convert / das_execute only enqueue work on the given CUDA stream (a cudaStream_t
  *     passed as void*; NULL = the legacy default stream).  They never synchronise and never
- *     allocate.  A plan is immutable after creation: concurrent das_execute calls on
- *     different streams with different buffers are allowed.
+ *     allocate.  A plan's geometry and launch shapes never change after creation: concurrent das_execute
+ *     calls on different streams with different buffers are allowed (a DAS_ALGO_TC plan also owns pacing words
+ *     that its launches write; see das_execute).
  */
 #ifndef DAS_B200_H_
 #define DAS_B200_H_
@@ -53,9 +54,13 @@ typedef enum { DAS_DATA_IQ = 0, DAS_DATA_RF = 1 } das_data_kind_t;
 typedef enum {
   DAS_STORE_FP32 = 0,
   DAS_STORE_FP16 = 1,    /* the paper's mixed-precision storage */
-  DAS_STORE_FP8 = 2      /* e4m3, round to nearest even, saturating ("FP8 storage"): one frame per
-                            call, general and tiled kernels; the caller's `scale` must bring the data into the
-                            e4m3 range (|v| <= 448, resolution 2^-9 near zero); DESIGN.md gives the image quality */
+  DAS_STORE_FP8 = 2      /* e4m3, round to nearest even, saturating ("FP8 storage"): general and tiled
+                            kernels (n_frames > 1 runs frame by frame; DAS_ALGO_TC refuses it).  What is stored is
+                            the interval table (mid, slope) = ((y_k + y_k+1)/2, y_k+1 - y_k) of the scaled data, so
+                            the caller's `scale` must bring BOTH into the e4m3 range: |y_k| <= 448 and
+                            |y_k+1 - y_k| <= 448 (two neighbours of opposite sign near full scale break the
+                            second); a larger slope is clipped to +-448 without an error and that interval is then
+                            interpolated wrongly.  Resolution 2^-9 near zero; DESIGN.md gives the image quality */
 } das_storage_t;
 /* Receive window on the f-number cone ("receive weight ... origin and a direction"; DESIGN.md
  * reading W1).  With u = 2 f# rho / a in [0, 1] the normalised radius inside the cone:
@@ -140,7 +145,10 @@ int    das_plan_frames(const das_plan_t* plan);      /* B (>= 1)                
  *   d_conv  device, das_converted_bytes() bytes, 16-byte aligned; written entirely
  *   scale   every sample is multiplied by it before the cast (1.0f = none); lets the caller
  *           keep fp16 storage inside its normal range
- * fp16 storage rounds to nearest even; overflow gives +-inf (reading A11). */
+ * fp16 storage rounds to nearest even; overflow gives +-inf (reading A11).  The one-frame kernels read a
+ * sample only for the terms that use it, so an infinite sample spoils only the voxels whose sum contains it (as
+ * in the definition).  DAS_ALGO_TC multiplies whole sample windows by weight rows that are zero where a voxel does
+ * not use a sample, and 0 * inf = NaN: there the scaled data must stay finite in FP16 (|scale * y| < 65504). */
 das_status_t das_convert(const das_plan_t* plan, const void* d_raw, void* d_conv, float scale,
                          void* stream);
 
@@ -155,7 +163,9 @@ das_status_t das_convert(const das_plan_t* plan, const void* d_raw, void* d_conv
  * Calls on one plan may overlap (different streams, different buffers).  For DAS_ALGO_TC the CTAs of a launch pace
  * each other through progress words owned by the plan (L2 reuse between neighbouring tiles): overlapping launches
  * of ONE such plan stay correct (the pacing is advisory and its waits are bounded) but lose the pacing's benefit;
- * use one plan per stream. */
+ * use one plan per stream.  A launch whose CTAs are not all resident at once (an SM limit, MIG, a kernel of another
+ * stream holding SMs) also stays correct: a CTA waits for an absent partner for a few ms per launch at most (the
+ * wait budget shrinks each time it runs out), on top of the serialisation the missing SMs cause anyway. */
 das_status_t das_execute(const das_plan_t* plan, const void* d_conv, void* d_out, void* stream);
 
 /* End-to-end convenience for HOST buffers: copies h_raw to the device, runs das_convert

@@ -106,3 +106,37 @@ def test_fp8_rf_and_refusals(das_lib):
     with pytest.raises(das.DasError) as ei:                                # the tensor-core batch kernel pairs fp16 samples with fp16 weights
         das.Plan.from_workload(_cfg(1), storage=das.STORE_FP8, algo=das.ALGO_TC, n_frames=8)
     assert ei.value.status == das.ERR_UNSUPPORTED
+
+
+@pytest.mark.parametrize("algo", [1, 2])
+def test_fp8_slope_bound_and_saturation(das_lib, algo):
+    """include/das.h, DAS_STORE_FP8: the stored slope y_k+1 - y_k must fit e4m3 as well as the samples (ADVICE, round 2).
+    Neighbours of opposite sign near full scale: element 0 alternates +-200 (slopes +-400, inside the range: the
+    kernels must evaluate that table exactly as written), element 1 alternates +-300 (slopes +-600: the cast
+    saturates them to +-448, the documented clipping, and the kernels evaluate the clipped table)."""
+    import oracle.brute as brute
+    das = das_lib
+    q, m, k = 1, 2, 48
+    sign = np.where(np.arange(k) % 2 == 0, 1.0, -1.0)
+    y = np.zeros((q, m, k), np.complex64)
+    y[0, 0] = (200.0 * sign + 25.0j * sign).astype(np.complex64)
+    y[0, 1] = (300.0 * sign - 40.0j).astype(np.complex64)
+    w = wl.custom(wl.matrix_array(3)[:m], [wl.TX_PLANE], [[0, 0, 1]], [0.0], [-0.2e-3, 0.1e-3], [0.0], [0.8e-3, 1.0e-3, 1.3e-3],
+                  fs=15.6e6, n_samples=k, f_number=0.0, y=y)
+    got, used, conv = gpu_das(das, w, das.STORE_FP8, algo, return_conv=True)
+    assert used == algo
+    tab32 = expected_table(y, wl.DATA_IQ, 0)                            # [M, Q, Kp, (mid|slope), comp] float32
+    assert np.abs(tab32[0]).max() == 400.0 and np.abs(tab32[1]).max() == 600.0
+    want = e4m3_bytes(np.clip(tab32, -448.0, 448.0)).reshape(-1)
+    same = (conv == want) | (((conv | want) & 0x7f) == 0)
+    assert same.all(), f"{(~same).sum()} of {want.size} bytes differ"
+    yf = y.view(np.float32).reshape(y.shape + (2,))
+    mid = e4m3(yf[:, :, :-1] * np.float32(0.5) + yf[:, :, 1:] * np.float32(0.5))
+    slope = e4m3(np.clip(yf[:, :, 1:] - yf[:, :, :-1], -448.0, 448.0))
+    ref = brute.das_from_interval_table(w, mid[..., 0] + 1j * mid[..., 1], slope[..., 0] + 1j * slope[..., 1])
+    emax, _ = errors(got, ref)
+    assert emax <= 1e-5, f"fp8 table with saturated slopes: max error {emax:.3e}"
+    # and the clipping is a real loss: against the unclipped table the volume is off by far more than the gate
+    slope_true = yf[:, :, 1:] - yf[:, :, :-1]
+    full = brute.das_from_interval_table(w, mid[..., 0] + 1j * mid[..., 1], slope_true[..., 0] + 1j * slope_true[..., 1])
+    assert errors(got, full)[0] > 1e-2
