@@ -157,6 +157,9 @@ int das_oracle_ex(const float* elem_pos, const float* elem_dir, int M,
       if (q < 0 || q >= Q) { bad = 1; continue; }
       const double vx = (double)tx_v[3 * q], vy = (double)tx_v[3 * q + 1], vz = (double)tx_v[3 * q + 2];
       const double w_tx = o->w_tx_tab ? (double)o->w_tx_tab[(size_t)q * (size_t)n_total + (size_t)n] : 1.0;
+      /* reading W5 ("skip these negligible contributions"): a transmit weight of
+         exactly 0 is the same as not listing the transmit -- its samples are never read and its terms not counted */
+      if (w_tx == 0.0) continue;
       double tau_tx;
       if (o->tau_tx_tab) {
         tau_tx = (double)o->tau_tx_tab[(size_t)q * (size_t)n_total + (size_t)n];

@@ -500,6 +500,7 @@ tiled_kernel(const TiledDev tp, const Params P, const unsigned char* __restrict_
       for (int j = 0; j < 2 * QP; ++j) {
         if (j < QC && q0 + j < P.Q) {
           const float wq = GEN ? tx_weight(P, q0 + j, n_flat) : 1.f;        // transmit weight (1 without a table)
+          if (GEN && wq == 0.f) continue;      // reading W5: weight 0 = not listed; what its samples gave (inf, NaN) is dropped
           if (IQ) {
             const float ang = 6.283185307179586f * sm.cyc[IQ ? j : 0][tid];
             const float cs = wq * cos_approx(ang), sn = wq * sin_approx(ang);

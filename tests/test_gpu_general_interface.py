@@ -183,3 +183,35 @@ def test_tc_kernel_tilted_normals(das_lib):
             emax, el2 = errors(g_[b], ref)
             assert emax <= TOL_FP16_MAX and el2 <= TOL_FP16_L2, (b, kw, emax, el2)
     assert np.abs(oracle.das(w) - oracle.das(base)).max() > 0.01 * np.abs(oracle.das(base)).max()   # the tilts matter
+
+
+@pytest.mark.parametrize("algo", [1, 2])
+def test_unlisted_transmit_is_never_summed(das_lib, algo):
+    """Reading W5: a transmit a voxel does not list -- or lists with weight 0 --
+    contributes nothing, whatever its samples hold.  Transmit 2 of config 2 is listed by no voxel and its traces
+    are full of +-inf (reading A11 lets fp16 overflow to inf): the volume must equal the oracle's, finite, and the
+    term count (das_plan_count_work, the roofline's unit) must equal the oracle's count with the zeros left out."""
+    import oracle
+    das = das_lib
+    torch = _torch()
+    w = _cfg(2, (20, 18, 24))
+    n, q_n = w.n_voxels, w.n_tx
+    rng = np.random.default_rng(8)
+    mask = rng.random((q_n, n)) < 0.7
+    mask[2] = False
+    mask[0, ~mask.any(axis=0)] = True
+    off = np.concatenate([[0], np.cumsum(mask.sum(0))]).astype(np.int64)
+    oq = np.concatenate([np.nonzero(mask[:, i])[0] for i in range(n)]).astype(np.int32)
+    wt = np.where(rng.random((q_n, n)) < 0.2, 0.0, rng.uniform(0.5, 1.5, (q_n, n))).astype(np.float32)   # explicit zeros too
+    y = w.y.copy()
+    y[2, :, ::3] = np.inf
+    y[2, :, 1::3] = -np.inf
+    ref = oracle.das(w, y=y, w_tx=wt, obs=(off, oq), want_count=True)
+    assert np.isfinite(ref["out"]).all()
+    for storage in (das.STORE_FP32, das.STORE_FP16):
+        got = run(das, w, storage, algo, algo, y=y, w_tx=wt, obs=(off, oq))
+        assert np.isfinite(got.view(np.float32)).all(), "an unlisted transmit leaked into the sum"
+        check(got, ref["out"], storage, das, "unlisted transmit with infinite samples")
+    plan = das.Plan.from_workload(w, storage=das.STORE_FP32, algo=algo, w_tx=wt, obs=(off, oq))
+    assert plan.count_work()[1] == int(ref["count"].sum())
+    plan.destroy()

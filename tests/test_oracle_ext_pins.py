@@ -92,6 +92,32 @@ def test_unit_weights_and_full_lists_reduce_to_the_plain_oracle(oracle):
     assert np.all(z == 0)
 
 
+def test_zero_weight_equals_not_listed(oracle):
+    """Reading W5: w_tx == 0 is the same as not listing the transmit.  A weight
+    table with explicit zeros gives the volume AND the term count of the observation lists that leave those
+    (q, n) out, bit for bit, and an infinite sample in a zero-weighted transmit is never read."""
+    w = _small_problem(14)
+    n = w.n_voxels
+    rng = np.random.default_rng(2)
+    keep = rng.random((2, n)) < 0.6                                   # which (q, n) stay
+    keep[:, 0] = [False, False]                                       # one voxel with nothing left
+    wt = np.where(keep, rng.uniform(0.5, 1.5, (2, n)), 0.0).astype(np.float32)
+    off = np.concatenate([[0], np.cumsum(keep.sum(axis=0))])
+    oq = np.concatenate([np.nonzero(keep[:, i])[0] for i in range(n)]).astype(np.int32)
+    a = oracle.das(w, w_tx=wt, want_count=True)
+    b = oracle.das(w, w_tx=np.where(keep, wt, 7.0).astype(np.float32), obs=(off, oq), want_count=True)
+    assert np.array_equal(a["out"], b["out"]) and np.array_equal(a["count"], b["count"])
+    full = oracle.das(w, want_count=True)
+    assert 0 < a["count"].sum() < full["count"].sum() and a["count"].ravel()[0] == 0 and a["out"].ravel()[0] == 0
+    # transmit 1 switched off everywhere: its samples may hold anything
+    y = w.y.copy()
+    y[1, :, ::7] = np.inf
+    wt1 = np.stack([np.ones(n, np.float32), np.zeros(n, np.float32)])
+    got = oracle.das(w, y=y, w_tx=wt1)
+    assert np.isfinite(got).all()
+    assert np.array_equal(got, oracle.das(w, obs=(np.arange(n + 1), np.zeros(n, np.int32))))
+
+
 def test_weights_scale_each_transmit(oracle):
     """x = sum_q w_q x_q for weights constant over the voxels (linearity in w_tx)."""
     w = _small_problem(12)
