@@ -58,6 +58,8 @@ UNIT = "volumes/s"
 FLOPS_PER_TERM = {0: 17.0, 1: 8.0}
 FLOPS_PER_PAIR = 28.0
 FP32_LANES_PER_SM = 128          # B200_PROFILING.md / B300_MICROARCH.md: 4 SMSP x 32 lanes
+SMEM_BYTES_PER_CLK_PER_SM = 128  # shared-memory data pipe: one 128-byte wavefront per SM per clock
+SMEM_BYTES_PER_TERM = 8.0        # the (mid, slope) entry of one term in fp16 storage (16 for fp32 IQ)
 N_SM = 148
 
 PROFILES = os.path.join(ROOT, "profiles")
@@ -101,6 +103,8 @@ def parse_args():
     ap.add_argument("--frames", type=int, default=4,
                     help="distinct raw frames rotated through the timed steps (inputs > L2)")
     ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--no-extras", action="store_true",
+                    help="skip the other_configs / general_interface legs of the default run")
     ap.add_argument("--cpu-seconds", type=float, default=15.0,
                     help="target CPU time of the cpu_baseline oracle sample (0 = skip)")
     return ap.parse_args()
@@ -299,6 +303,30 @@ def fp32_peak_tflops(sampler_max_mhz):
     return N_SM * FP32_LANES_PER_SM * 2 * mhz * 1e6 / 1e12, f"148 SM x 128 lanes x 2 flop x {mhz:.0f} MHz ({src})"
 
 
+def sm_max_mhz(sampler_max_mhz):
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["sm_max_mhz"])
+    except Exception:
+        return float(sampler_max_mhz) if sampler_max_mhz else 1965.0
+
+
+def ncu_static(prof, default_bound, measured_ms):
+    """Counters of a COMMITTED ncu capture (profiles/*.json): context for the measured roofline, never the roofline
+    itself.  `stale` says that the capture's kernel time differs from this run's by more than 10 %, i.e. the kernel
+    has changed since it was profiled (or the clocks differ) and the counters describe another binary."""
+    if not prof:
+        return None
+    d = {k: prof[k] for k in ("utilisation_pct", "dram_bytes", "dram_bytes_read", "dram_bytes_write", "l2_hit_rate_pct",
+                              "warp_instructions", "gpu_time_ms", "kernel", "source", "command") if k in prof}
+    d["binding_counter"] = dict(zip(("name", "pct"), bound_from_profile(prof, default_bound)))
+    t = prof.get("gpu_time_ms")
+    d["measured_kernel_ms_this_run"] = measured_ms
+    d["stale"] = bool(t is None or abs(float(t) - measured_ms) > 0.10 * measured_ms)
+    d["note"] = "from a committed capture, not re-measured in this run; utilisation is pipe-busy time, not work done"
+    return d
+
+
 def tensor_peak_tflops():
     """Dense FP16 tensor peak from MEASURED_PEAKS.json (driver-written, bf16 cuBLAS; FP16 and BF16 run at the
     same rate).  The batch kernel is timed inside a long, power-capped step loop, so the denominator is the
@@ -334,6 +362,71 @@ def time_loop(torch, stream, step, steps, warmup, barrier, max_over_ranks, local
     conv_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
     exec_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
     return total_ms, conv_ms, exec_ms, launches, cs.summary()
+
+
+def measure_one_frame(torch, das, dev, stream, w, storage_name, steps, warmup, plan_options=None, flush=None):
+    """One frame per call on workload `w`: das_convert + das_execute timed per step with CUDA events on `stream`;
+    a 256 MB buffer is rewritten between the steps (outside the event pairs) so that no step finds its input in L2
+    (configs 1 and 2 are smaller than L2).  Returns the dict of one `other_configs` / `general_interface` entry."""
+    storage = das.STORE_FP16 if storage_name == "fp16" else das.STORE_FP32
+    plan = das.Plan.from_workload(w, storage=storage, algo=das.ALGO_AUTO, device=dev.index, **(plan_options or {}))
+    kernel = {das.ALGO_GENERAL: "general", das.ALGO_TILED: "tiled"}[plan.algo]
+    n_pairs, n_terms = plan.count_work()
+    raws = [torch.from_numpy(np.ascontiguousarray(f)).to(dev) for f in make_frames(w, 2)]
+    out = torch.empty(w.grid_shape, dtype=torch.complex64 if w.data_kind == 0 else torch.float32, device=dev)
+    conv = torch.empty(plan.converted_bytes, dtype=torch.uint8, device=dev)
+    sp = stream.cuda_stream
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+    n0 = das.launch_count()
+    for i in range(warmup + steps):
+        if flush is not None:
+            with torch.cuda.stream(stream):
+                flush.zero_()
+        ev = evs[i - warmup] if i >= warmup else None
+        if ev:
+            ev[0].record(stream)
+        plan.convert(raws[i % 2].data_ptr(), conv.data_ptr(), 1.0, sp)
+        if ev:
+            ev[1].record(stream)
+        plan.execute(conv.data_ptr(), out.data_ptr(), sp)
+        if ev:
+            ev[2].record(stream)
+    stream.synchronize()
+    conv_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    exec_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+    step_ms = float(np.mean([e[0].elapsed_time(e[2]) for e in evs]))
+    flops = FLOPS_PER_TERM[w.data_kind] * n_terms + FLOPS_PER_PAIR * n_pairs
+    peak, _ = fp32_peak_tflops(None)
+    ach = flops / (exec_ms * 1e-3) / 1e12
+    res = {"workload": workload_name(w, storage_name), "kernel": kernel, "value": 1e3 / step_ms, "unit": UNIT,
+           "ms_per_step": step_ms, "steps": steps, "kernels_ms": {"das_convert": conv_ms, "das_execute": exec_ms},
+           "entered_terms_per_volume": n_terms, "gpu_launches": int(das.launch_count() - n0),
+           "roofline": {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                        "flops_per_launch": flops},
+           "l2": "256 MB written between steps (L2 flush), outside the timed event pairs"}
+    plan.destroy()
+    return res
+
+
+def general_interface_tables(w):
+    """The paper's general interface on the headline geometry: tau_tx as a [Q][N] table that
+    restates the diverging-wave model, and a smooth transmit weight w_tx (a Gaussian of the lateral distance
+    from the virtual source, sigma 6 mm: the transmit field's magnitude)."""
+    gx, gy, gz = np.meshgrid(w.xs.astype(np.float64), w.ys.astype(np.float64), w.zs.astype(np.float64), indexing="ij")
+    tau = np.empty((w.n_tx, gx.size), np.float32)
+    wt = np.empty((w.n_tx, gx.size), np.float32)
+    for q in range(w.n_tx):
+        v = w.tx_v[q].astype(np.float64)
+        if int(w.tx_type[q]) == 0:
+            t = (gx * v[0] + gy * v[1] + gz * v[2]) / w.c + float(w.tx_t0[q])
+            lat2 = np.zeros_like(gx)
+        else:
+            t = np.sqrt((gx - v[0]) ** 2 + (gy - v[1]) ** 2 + (gz - v[2]) ** 2) / w.c + float(w.tx_t0[q])
+            lat2 = (gx - v[0]) ** 2 + (gy - v[1]) ** 2
+        tau[q] = t.ravel().astype(np.float32)
+        wt[q] = np.exp(-lat2 / (2.0 * 6e-3 ** 2)).ravel().astype(np.float32)
+    return tau, wt
+
 
 
 def run_cuda(args):
@@ -475,6 +568,25 @@ def run_cuda(args):
     h2d_ms = h_beg.elapsed_time(h_end)
     checksum = float(h_out.abs().max())                                   # the D2H result is read
 
+    # ---- the other BASELINE.json configs and the general interface, one frame per call (single GPU, default run)
+    other, gen_if = None, None
+    if world == 1 and args.config == 3 and not args.no_extras:
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+        other = []
+        for number, st in ((1, "fp16"), (2, "fp16"), (4, "fp16"), (4, "fp32")):
+            wo = wl.config(number)
+            other.append(dict({"config": number}, **measure_one_frame(torch, das, dev, stream, wo, st, 10, 3, flush=flush)))
+            del wo
+        if args.storage == "fp16":
+            tau, wt = general_interface_tables(w)
+            gen_if = measure_one_frame(torch, das, dev, stream, w, "fp16", 10, 3, plan_options={"tau_tx": tau, "w_tx": wt}, flush=flush)
+            gen_if["tables"] = {"tau_tx_bytes": int(tau.nbytes), "w_tx_bytes": int(wt.nbytes),
+                                "what": "tau_tx restates the diverging-wave delays as a [Q][N] table; w_tx is a Gaussian of the "
+                                        "lateral distance from the virtual source (sigma 6 mm)"}
+            gen_if["analytic_path_execute_ms"] = exec1
+            del tau, wt
+        del flush
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -504,10 +616,8 @@ def run_cuda(args):
     extra = {}
     traffic = None
     if prof:
-        traffic = prof.get("dram_bytes")
-        extra = {"ncu": {k: prof[k] for k in ("utilisation_pct", "dram_bytes_read", "dram_bytes_write", "l2_hit_rate_pct",
-                                                "warp_instructions", "gpu_time_ms", "kernel", "source", "command") if k in prof}}
-        extra["ncu"]["binding_counter"] = dict(zip(("name", "pct"), bound_from_profile(prof, bound)))
+        traffic = prof.get("dram_bytes")          # per launch, from the ncu --set full capture named in ncu_static.source
+        extra = {"ncu_static": ncu_static(prof, bound, exec_ms)}
     achieved = flops / (exec_ms * 1e-3) / 1e12
     raw_bytes = sum(r.nbytes for r in raws)
     line = {
@@ -545,20 +655,25 @@ def run_cuda(args):
     }
     sf = line["single_frame"]["roofline"]
     sf["frac"] = sf["achieved"] / sf["peak"]
+    sf["flops_per_launch"] = flops1
+    sf["peak_how"] = fp32_peak_tflops(clocks.get("sm_max_mhz"))[1] + ", derived (no measured FP32 peak)"
+    # the same launch on the shared-memory roofline (the pipe ncu shows busiest for the tiled kernel): ALGORITHMIC bytes,
+    # one (mid, slope) entry per entered term, against 148 SM x 128 B/clk.  What the kernel really moves through
+    # that pipe is more (a 16-byte line-table entry read by LDS.128 = four wavefronts per warp instruction).
+    if algo1 == "tiled":
+        ent = SMEM_BYTES_PER_TERM * (2.0 if args.storage == "fp32" else 1.0) * (1.0 if w.data_kind == 0 else 0.5)
+        smem_peak = N_SM * SMEM_BYTES_PER_CLK_PER_SM * sm_max_mhz(clocks.get("sm_max_mhz")) * 1e6 / 1e12
+        smem_ach = ent * n_terms / (exec1 * 1e-3) / 1e12
+        sf["smem_roofline"] = {"bound": "shared-memory bandwidth", "achieved": smem_ach, "peak": smem_peak, "unit": "TB/s",
+                               "frac": smem_ach / smem_peak, "bytes_per_term": ent,
+                               "peak_how": "148 SM x 128 B/clk x max SM clock, derived"}
     if prof_tiled and algo1 == "tiled":
-        # the binding roofline of the one-frame kernel is the largest utilisation counter of its capture
-        name, pct = bound_from_profile(prof_tiled, "alu")
-        sf["binding_counter"] = {"name": name, "pct": pct, "source": prof_tiled["source"]}
+        sf["ncu_static"] = ncu_static(prof_tiled, "alu", exec1)
         sf["traffic"] = prof_tiled.get("dram_bytes")
-        # the bound is the pipe ncu shows busiest (the shared-memory wavefront pipe: one LDS.128 per term costs four
-        # wavefronts); the FP32-ALU figures stay beside it as `alu_roofline`
-        sf["alu_roofline"] = {k: sf[k] for k in ("achieved", "peak", "unit", "frac")}
-        sf["bound"] = name
-        sf["achieved"], sf["peak"], sf["unit"] = pct, 100.0, "% of the pipe's peak (ncu)"
-        sf["frac"] = pct / 100.0
-        sf["frac_how"] = "ncu utilisation of the binding pipe in the committed capture (not re-measured in this run)"
     # both readings of the metric at top level: B frames per call (value) and one frame per call
     line["value_frames_per_call"] = B
+    line["other_configs"] = other
+    line["general_interface"] = gen_if
     line["value_one_frame_per_call"] = line["single_frame"]["value"]
     if world == 1 and args.cpu_seconds > 0:
         line["cpu_baseline"] = cpu_baseline(w, args.cpu_seconds)
