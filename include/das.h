@@ -115,7 +115,9 @@ typedef struct {
    *      pointers, copied at plan creation.  N = nx*ny*nz, voxel order = output order. ---- */
   const float* tau_tx;      /* [Q][N] transmit delays tau_tx_qn in seconds; when given they
                                replace the delay models of tx[] (type / v / t0 are then ignored) */
-  const float* w_tx;        /* [Q][N] transmit weights w_tx_qn (magnitude of the transmit field) */
+  const float* w_tx;        /* [Q][N] transmit weights w_tx_qn (magnitude of the transmit field).  A weight of
+                               exactly 0 means the same as voxel n not listing transmit q (below): the samples of that
+                               (q, n) are not summed, whatever they hold, and das_plan_count_work does not count them */
   const long long* obs_off; /* [N+1] CSR offsets of the per-voxel observation lists: voxel n sums */
   const int* obs_q;         /* [obs_off[N]] only over the transmits listed for it, each at most once */
   const float* vox_pos;     /* [N][3] an arbitrary voxel list ("{p_n}") instead of the grid axes:
@@ -123,6 +125,11 @@ typedef struct {
   int   window;             /* das_window_t */
   float window_param;       /* TUKEY: taper fraction b in (0, 1] */
   int   interp;             /* das_interp_t; CUBIC: general kernel only, one frame per call */
+  /* ---- debugging aids; 0 = the library's choice.  They change launch shapes, never results (tests use them to
+   *      force a ragged grid of CTAs and to compare paced with unpaced launches).  The library reads no
+   *      environment variable unless it is built with -DDAS_TUNING (kernel-tuning sweeps). ---- */
+  int   debug_tiled_grid;   /* CTAs of the one-frame tiled kernel (default: one or two per SM, at most one per tile) */
+  int   debug_tc_pace;      /* DAS_ALGO_TC quad pacing (das_execute): lead in receivers, default 16; -1 = no pacing */
 } das_plan_desc_t;
 
 /* The problem statement of PAPER.md:29-50 (Eq. 1: delays; Eq. 2: the weighted sum; linear interpolation) and

@@ -58,6 +58,7 @@ class PlanDesc(ctypes.Structure):
         ("obs_off", ctypes.POINTER(ctypes.c_longlong)), ("obs_q", ctypes.POINTER(ctypes.c_int)),
         ("vox_pos", ctypes.POINTER(ctypes.c_float)),
         ("window", ctypes.c_int), ("window_param", ctypes.c_float), ("interp", ctypes.c_int),
+        ("debug_tiled_grid", ctypes.c_int), ("debug_tc_pace", ctypes.c_int),
     ]
 
 
@@ -150,7 +151,7 @@ class Plan:
     def __init__(self, elem_pos, tx_type, tx_v, tx_t0, xs, ys, zs, *, c, fc, fs, t_start=0.0,
                  f_number=1.0, n_samples, data_kind=DATA_IQ, storage=STORE_FP32, algo=ALGO_AUTO,
                  device=0, elem_dir=None, n_frames=0, tau_tx=None, w_tx=None, obs=None, vox_pos=None,
-                 window=WINDOW_BOXCAR, window_param=0.5, interp=INTERP_LINEAR):
+                 window=WINDOW_BOXCAR, window_param=0.5, interp=INTERP_LINEAR, debug_tiled_grid=0, debug_tc_pace=0):
         lib = load()
         self._lib = lib
         self._h = ctypes.c_void_p()
@@ -197,6 +198,7 @@ class Plan:
         if vox_pos is not None:
             d.vox_pos = vox_pos.ctypes.data_as(fp); keep.append(vox_pos)
         d.window, d.window_param, d.interp = int(window), float(window_param), int(interp)
+        d.debug_tiled_grid, d.debug_tc_pace = int(debug_tiled_grid), int(debug_tc_pace)
         self.desc = d
         _check(lib.das_plan_create(ctypes.byref(d), ctypes.byref(self._h)))
         self.grid_shape = (len(xs), len(ys), len(zs))
@@ -206,7 +208,8 @@ class Plan:
     @classmethod
     def from_workload(cls, w, *, storage=STORE_FP32, algo=ALGO_AUTO, device=0, n_frames=0, **options):
         """Plan for a ``workloads.Workload``-shaped object (duck-typed); ``options`` are the keyword
-        arguments of the paper's general interface (tau_tx, w_tx, obs, vox_pos, window, window_param, interp)."""
+        arguments of the paper's general interface (tau_tx, w_tx, obs, vox_pos, window, window_param, interp) and
+        the debugging aids of das.h (debug_tiled_grid, debug_tc_pace)."""
         return cls(w.elem_pos, w.tx_type, w.tx_v, w.tx_t0, w.xs, w.ys, w.zs, c=w.c, fc=w.fc, fs=w.fs,
                    t_start=w.t_start, f_number=w.f_number, n_samples=w.n_samples,
                    data_kind=w.data_kind, storage=storage, algo=algo, device=device,

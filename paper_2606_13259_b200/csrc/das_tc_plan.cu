@@ -203,10 +203,12 @@ static TcPlan* tc_plan_create_groups(const Params& P, const das_plan_desc_t& d, 
       (e = cudaMemcpy(edge.data(), d_edge, sizeof(int) * n_tiles, cudaMemcpyDeviceToHost)) != cudaSuccess ||
       (e = cudaMemcpy(stats, d_stats, sizeof(stats), cudaMemcpyDeviceToHost)) != cudaSuccess) return fail(e);
   auto refuse_free = [&](const char* msg) -> TcPlan* { tc_plan_destroy(tp); return refuse(msg); };
+#ifdef DAS_TUNING
   if (getenv("DAS_TC_VERBOSE")) {
     long long tw = 0; for (int w_ : work) tw += w_;
     fprintf(stderr, "[das tc plan] tiles %d, list entries %zu, MMA passes %lld, widest item %d samples, error bits %d\n", n_tiles, list.size(), tw, stats[0], stats[1]);
   }
+#endif
   if (stats[1] & 1) return refuse_free("a sample window of a voxel group needs more than 2 MMA passes (grid too coarse)");
   if (stats[1] & 2) {
     *retry_narrow = groups > 1 && !(stats[1] & 1);
@@ -263,20 +265,27 @@ static TcPlan* tc_plan_create_groups(const Params& P, const das_plan_desc_t& d, 
   // (the producer and the MMA issuers are serial latency chains), and as many stages as shared memory holds
   // (boxes in flight = what covers the L2 / HBM latency of the TMA copies).
   dv.qs = std::min(8, Q);
-  if (const char* ev = getenv("DAS_TC_QS")) dv.qs = std::min(kTcMaxQs, std::max(1, atoi(ev)));                          // tuning sweeps only
+#ifdef DAS_TUNING
+  if (const char* ev = getenv("DAS_TC_QS")) dv.qs = std::min(kTcMaxQs, std::max(1, atoi(ev)));
+#endif
   while (dv.qs > 1 && tc_smem_bytes(Bc, dv.qs, kTcMinStages) > 200 * 1024) dv.qs /= 2;
   dv.n_stages = kTcMinStages;
   while (dv.n_stages < 6 && tc_smem_bytes(Bc, dv.qs, dv.n_stages + 1) <= 200 * 1024) ++dv.n_stages;
-  if (const char* ev = getenv("DAS_TC_STAGES")) dv.n_stages = std::min(kTcMaxStages, std::max(kTcMinStages, atoi(ev)));   // tuning sweeps only
+#ifdef DAS_TUNING
+  if (const char* ev = getenv("DAS_TC_STAGES")) dv.n_stages = std::min(kTcMaxStages, std::max(kTcMinStages, atoi(ev)));
+#endif
   while (dv.n_stages > kTcMinStages && tc_smem_bytes(Bc, dv.qs, dv.n_stages) > 200 * 1024) --dv.n_stages;
   tp->smem = tc_smem_bytes(Bc, dv.qs, dv.n_stages);
   if (tp->smem > 200 * 1024) return refuse_free("stage ring does not fit in shared memory");
   tp->grid = std::max(4, std::min(dv.n_tiles * dv.n_chunks, prop.multiProcessorCount) / 4 * 4);
-  // quad pacing: one progress word per CTA (DAS_TC_PACE = 0 switches it off, any other value sets the lead in receivers)
-  dv.pace = 16;
-  if (const char* ev = getenv("DAS_TC_PACE")) dv.pace = atoi(ev);                                                        // tuning sweeps only
+  // quad pacing: one progress word per CTA; the lead in receivers is 16 unless the descriptor's debug field says
+  // otherwise (-1 = no pacing)
+  dv.pace = d.debug_tc_pace > 0 ? d.debug_tc_pace : (d.debug_tc_pace < 0 ? 0 : 16);
   dv.pace_mask = 3;
-  if (const char* ev = getenv("DAS_TC_PACE_MASK")) dv.pace_mask = atoi(ev);                                             // tuning sweeps only
+#ifdef DAS_TUNING
+  if (const char* ev = getenv("DAS_TC_PACE")) dv.pace = atoi(ev);
+  if (const char* ev = getenv("DAS_TC_PACE_MASK")) dv.pace_mask = atoi(ev);
+#endif
   dv.progress = nullptr;
   dv.epoch = 0;
   if (dv.pace > 0) {

@@ -192,8 +192,10 @@ TiledPlan* tiled_plan_create(const Params& P, const das_plan_desc_t& d, int devi
   const size_t smem = tiled_smem_bytes(QC, W, P.iq, st);
   const int ctas_per_sm = (smem + 1024) * 2 <= (size_t)prop.sharedMemPerMultiprocessor ? 2 : 1;
   tp->grid = std::max(1, std::min(n_tiles, prop.multiProcessorCount * ctas_per_sm));
-  if (const char* ev = getenv("DAS_TILED_GRID")) tp->grid = std::max(1, std::min(n_tiles, atoi(ev)));   // debugging only
+  if (d.debug_tiled_grid > 0) tp->grid = std::max(1, std::min(n_tiles, d.debug_tiled_grid));      // das.h: debugging aid
+#ifdef DAS_TUNING
   if (getenv("DAS_TC_VERBOSE")) fprintf(stderr, "[das tiled plan] tiles %d, QC %d, W %d, smem %zu, grid %d\n", n_tiles, QC, W, smem, tp->grid);
+#endif
   TiledDev& dv = tp->dev;
   dv.n_tiles = n_tiles;
   dv.n_chunks = (Q + QC - 1) / QC;

@@ -390,7 +390,7 @@ def test_count_work_out_of_range(das_lib):
 
 
 @pytest.mark.timeout(180)
-def test_tiled_kernel_repeated_launches_do_not_hang(das_lib, monkeypatch):
+def test_tiled_kernel_repeated_launches_do_not_hang(das_lib):
     """Regression (round 2): with 3 converter warps over 4-deep rings a converter could fall through the parity wait
     of a slot whose previous round was still in flight; about one launch in fifty of the RF fp32 headline then
     deadlocked its mbarrier rings (found with cuda-gdb: all three roles of one CTA parked in try_wait).  The rings
@@ -399,9 +399,8 @@ def test_tiled_kernel_repeated_launches_do_not_hang(das_lib, monkeypatch):
     the last result with the first (the kernel is deterministic)."""
     torch = _torch()
     das = das_lib
-    monkeypatch.setenv("DAS_TILED_GRID", "74")
     w = wl.config(4, generate_data=False)
-    plan = das.Plan.from_workload(w, storage=das.STORE_FP32, algo=das.ALGO_TILED)
+    plan = das.Plan.from_workload(w, storage=das.STORE_FP32, algo=das.ALGO_TILED, debug_tiled_grid=74)
     g = torch.Generator(device="cuda").manual_seed(3)
     raw = torch.randn((w.n_tx, w.n_elem, w.n_samples), device="cuda", generator=g)
     conv = torch.empty(plan.converted_bytes, dtype=torch.uint8, device="cuda")

@@ -282,9 +282,9 @@ def test_tc_repeated_launches_deterministic(das_lib):
     plan.destroy()
 
 
-def test_tc_quad_pacing_does_not_change_results(das_lib, monkeypatch):
-    """The producers' quad pacing only delays TMA copies: with it switched off (DAS_TC_PACE=0 at plan
-    creation) the output must be bit-identical.  Config 2 geometry, ragged sub-grid (rim quads are filled up with
+def test_tc_quad_pacing_does_not_change_results(das_lib):
+    """The producers' quad pacing only delays TMA copies: with it switched off (debug_tc_pace = -1 in
+    the plan descriptor) the output must be bit-identical.  Config 2 geometry, ragged sub-grid (rim quads are filled up with
     empty tiles), 16 frames."""
     torch = _torch()
     das = das_lib
@@ -292,14 +292,14 @@ def test_tc_quad_pacing_does_not_change_results(das_lib, monkeypatch):
     g = torch.Generator(device="cuda").manual_seed(11)
     raw = torch.view_as_complex(torch.randn((16, w.n_tx, w.n_elem, w.n_samples, 2), device="cuda", generator=g) * 0.1)
     outs = []
-    for pace in ("0", "16"):
-        monkeypatch.setenv("DAS_TC_PACE", pace)
-        plan = das.Plan.from_workload(w, storage=das.STORE_FP16, algo=das.ALGO_TC, n_frames=16)
+    for pace in (-1, 0, 4):                           # off, the default lead (16), a short lead
+        plan = das.Plan.from_workload(w, storage=das.STORE_FP16, algo=das.ALGO_TC, n_frames=16, debug_tc_pace=pace)
         out, _ = das.beamform_torch(plan, raw)
         torch.cuda.synchronize()
         outs.append(out.clone())
         plan.destroy()
     assert torch.equal(torch.view_as_real(outs[0]), torch.view_as_real(outs[1]))
+    assert torch.equal(torch.view_as_real(outs[0]), torch.view_as_real(outs[2]))
 
 
 def test_tc_pacing_gives_up_on_a_partner_that_is_not_resident(das_lib):
