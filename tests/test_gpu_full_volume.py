@@ -48,7 +48,8 @@ _memo = {}
 
 
 def oracle_full_cached(number):
-    """(out [nx,ny,nz] complex128 / float64, l1 [nx,ny,nz] float64) of oracle.das on config `number`."""
+    """(out [nx,ny,nz] complex128 / float64, l1 [nx,ny,nz] float64) of oracle.das on config `number`; the per-voxel
+    term counts of the same run are kept beside them (oracle_count_cached)."""
     if number in _memo:
         return _memo[number]
     import oracle
@@ -59,20 +60,30 @@ def oracle_full_cached(number):
     if os.path.exists(path):
         try:
             with np.load(path) as z:
-                if str(z["fingerprint"]) == fp:
-                    res = (z["out"], z["l1"])
+                if str(z["fingerprint"]) == fp and "count" in z.files:
+                    res = (z["out"], z["l1"], z["count"])
         except Exception:
             res = None
     if res is None:
-        r = oracle.das(w, want_l1=True)
-        res = (r["out"], r["l1"])
+        r = oracle.das(w, want_l1=True, want_count=True)
+        res = (r["out"], r["l1"], r["count"])
         try:
             os.makedirs(CACHE_DIR, exist_ok=True)
-            np.savez(path, out=res[0], l1=res[1], fingerprint=fp)
+            np.savez(path, out=res[0], l1=res[1], count=res[2], fingerprint=fp)
         except OSError:
             pass
-    _memo[number] = res
-    return res
+    _memo[number] = res[:2]
+    _memo_count[number] = res[2]
+    return res[:2]
+
+
+_memo_count = {}
+
+
+def oracle_count_cached(number):
+    """Per-voxel number of entered (q, m) terms of config `number` (the oracle's `count`, integer work)."""
+    oracle_full_cached(number)
+    return _memo_count[number]
 
 
 def check_p12(got, ref, l1, label):
@@ -119,6 +130,69 @@ def test_headline_full_volume_tc_batch8(das_lib):
     r5 = oracle.das(w, y=yb[5], voxels=vox)
     e5, l5 = errors(got[5].reshape(-1)[vox], r5)
     assert e5 <= TOL_FP16_MAX and l5 <= TOL_FP16_L2, (e5, l5)
+
+
+def test_headline_full_volume_tc_batch64(das_lib):
+    """The launch bench.py times (B = 64: MMA N = 128, 16 column groups per box), ALL 2 097 152 voxels of slot 0 = the
+    config's own data against the cached oracle volume (gates + P12 bound).  The other slots hold the same record under
+    exact power-of-two scales: FP16 rounding, the generated weights and FP32 accumulation all commute with such a
+    scale, so slot b must equal slot 0 times its scale on every voxel (a property that needs no oracle at this size).
+    The roofline's unit count rides along: das_plan_count_work of the batch plan = the oracle's term count."""
+    das, torch = das_lib, _torch()
+    w = _cfg(3)
+    ref, l1 = oracle_full_cached(3)
+    B = 64
+    plan = das.Plan.from_workload(w, storage=das.STORE_FP16, algo=das.ALGO_AUTO, n_frames=B)
+    assert plan.algo == das.ALGO_TC
+    y0 = torch.from_numpy(w.y).cuda()
+    raw = torch.empty((B,) + tuple(w.y.shape), dtype=torch.complex64, device="cuda")
+    scale = [2.0 ** (-(b % 5)) for b in range(B)]
+    for b in range(B):
+        raw[b] = y0 * scale[b]
+    out, _ = das.beamform_torch(plan, raw)
+    torch.cuda.synchronize()
+    got0 = out[0].cpu().numpy()
+    emax, el2 = check(got0, ref, das.STORE_FP16, das, "config3 full volume tc B=64 slot 0")
+    worst = check_p12(got0, ref, l1, "config3 full volume tc B=64 slot 0")
+    print(f"config3 full volume tc B=64 slot 0: max {emax:.3e}, L2 {el2:.3e}, worst P12 ratio {worst:.3f}")
+    peak = float(out[0].abs().max())
+    for b in (1, 18, 37, 63):
+        dev = float((out[b] - out[0] * scale[b]).abs().max())
+        assert dev <= 1e-6 * peak * scale[b], f"slot {b} is not slot 0 times {scale[b]}: {dev:.3e}"
+    assert plan.count_work()[1] == int(oracle_count_cached(3).sum())
+    plan.destroy()
+
+
+def test_headline_term_count_tiled(das_lib):
+    """das_plan_count_work -- the unit count under every roofline figure of bench.py -- at the headline size, against
+    the oracle's integer count (12 970 766 784 entered terms)."""
+    das = das_lib
+    plan = das.Plan.from_workload(_cfg(3), storage=das.STORE_FP16, algo=das.ALGO_TILED)
+    n_pairs, n_terms = plan.count_work()
+    cnt = oracle_count_cached(3)
+    assert n_terms == int(cnt.sum())
+    assert n_terms == n_pairs * 16                    # every active pair enters with all 16 transmits at this record length
+    plan.destroy()
+
+
+@pytest.mark.parametrize("storage", [0, 1])
+def test_config4_full_volume(das_lib, storage):
+    """BASELINE.json configs[3]: the RF variant at headline scale (K = 2048 real samples, no rotation), ALL voxels, in
+    both storage modes; fp16 also against the per-voxel P12 bound; the term count equals the oracle's."""
+    das = das_lib
+    w = _cfg(4)
+    ref, l1 = oracle_full_cached(4)
+    out, used = gpu_das(das, w, storage, das.ALGO_AUTO)
+    assert used == das.ALGO_TILED and out.shape == ref.shape and out.dtype == np.float32
+    emax, el2 = check(out, ref, storage, das, f"config4 full volume storage={storage}")
+    if storage == das.STORE_FP16:
+        worst = check_p12(out, ref, l1, "config4 full volume tiled fp16")
+        print(f"config4 full volume tiled fp16: max {emax:.3e}, L2 {el2:.3e}, worst P12 ratio {worst:.3f}")
+    else:
+        print(f"config4 full volume tiled fp32: max {emax:.3e}, L2 {el2:.3e}")
+        plan = das.Plan.from_workload(w, storage=storage, algo=das.ALGO_TILED)
+        assert plan.count_work()[1] == int(oracle_count_cached(4).sum())
+        plan.destroy()
 
 
 # ------------------------------------------------------------------ batch layout of das_convert (bit-exact)
