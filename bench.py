@@ -586,6 +586,33 @@ def run_cuda(args):
             gen_if["analytic_path_execute_ms"] = exec1
             del tau, wt
         del flush
+    sel = None
+    if world == 1 and args.config == 3 and B > 1 and not args.no_extras:
+        # a spatially selective sequence: every voxel lists the 4 of the 16 virtual sources of its own
+        # lateral quadrant; items (q, m, depth group) nobody in a tile lists get no box, no A tile and no MMA
+        gx, gy, _ = np.meshgrid(w.xs, w.ys, w.zs, indexing="ij")
+        mask = ((np.signbit(w.tx_v[:, 0])[:, None] == np.signbit(gx.ravel())[None, :]) &
+                (np.signbit(w.tx_v[:, 1])[:, None] == np.signbit(gy.ravel())[None, :]))          # [Q, N]
+        off = np.concatenate([[0], np.cumsum(mask.sum(0))]).astype(np.int64)
+        oq = np.nonzero(mask.T)[1].astype(np.int32)
+        plan_s = das.Plan.from_workload(w, storage=storage, algo=das.ALGO_AUTO, device=local_rank, n_frames=B, obs=(off, oq))
+        conv_s = torch.empty(plan_s.converted_bytes, dtype=torch.uint8, device=dev)
+        plan_s.convert(raws[0].data_ptr(), conv_s.data_ptr(), 1.0, sp)
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(5)]
+        for i in range(2 + len(evs)):
+            if i >= 2:
+                evs[i - 2][0].record(stream)
+            plan_s.execute(conv_s.data_ptr(), out.data_ptr(), sp)
+            if i >= 2:
+                evs[i - 2][1].record(stream)
+        stream.synchronize()
+        sel_ms = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+        sel = {"what": "every voxel lists the 4 of 16 virtual sources of its lateral quadrant (observation lists, PAPER.md:365)",
+               "kernel": "tensor-core batch" if plan_s.algo == das.ALGO_TC else "other", "frames_per_call": B,
+               "das_execute_ms": sel_ms, "dense_das_execute_ms": exec_ms, "speedup": exec_ms / sel_ms,
+               "listed_terms_fraction": float(mask.mean()), "steps": len(evs)}
+        plan_s.destroy()
+        del conv_s, mask, off, oq
 
     if rank != 0:
         if dist is not None:
@@ -674,6 +701,7 @@ def run_cuda(args):
     line["value_frames_per_call"] = B
     line["other_configs"] = other
     line["general_interface"] = gen_if
+    line["selective_lists"] = sel
     line["value_one_frame_per_call"] = line["single_frame"]["value"]
     if world == 1 and args.cpu_seconds > 0:
         line["cpu_baseline"] = cpu_baseline(w, args.cpu_seconds)

@@ -207,7 +207,10 @@ tc_kernel(const TcDev tp, const Params P, const __grid_constant__ CUtensorMap tm
   const int n_work = tp.n_tiles * tp.n_chunks;
   const long long n_vox = (long long)P.nx * P.ny * P.nz;
   const int ql = min(lane & 15, P.Q - 1);                    // the transmit this lane reads windows for
-  const bool q16 = P.Q == 16;
+  // 16 transmits and no weight table: every receiver of a group has all 16 items, so the A-slot phases are
+  // compile-time constants (Q16 path).  With a weight table single items may be missing (nobody lists them): the
+  // general path, which tracks the slots at run time, takes those plans.
+  const bool q16 = P.Q == 16 && P.wtx_tab == nullptr;
 
   // barrier addresses: taken once through an opaque move so that ptxas keeps them in registers instead of
   // rebuilding the shared-window base (S2UR + ULEA) at every use
@@ -598,6 +601,7 @@ __global__ void __launch_bounds__(kTcG * kTcRows)
 tc_window_kernel(const TcDev tp, const Params P, uint2* __restrict__ list, unsigned short* __restrict__ codes,
                  int* __restrict__ tile_work, int* __restrict__ tile_edge, int* __restrict__ stats) {
   __shared__ int kmn[kTcG][16], kmx[kTcG][16];
+  __shared__ unsigned lst[kTcG];                              // per group: transmits some active voxel lists, this receiver
   const int tile_i = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
   const int g = tid / kTcRows, row = tid % kTcRows;
   const TcTile td = tp.tiles[tile_i];
@@ -610,10 +614,19 @@ tc_window_kernel(const TcDev tp, const Params P, uint2* __restrict__ list, unsig
   }
   const int tb = tid < 16 ? __ldg(&tp.tbase[(long long)tile_i * P.Q + min(tid, P.Q - 1)]) : 0;
   int work = 0, edge = 0, span = 0, err = 0;
+  // transmits this voxel sums over: all of them, or those with a non-zero weight when the plan has a weight table
+  // (observation lists are stored as zeros of that table; reading W5).  An item (q, m, group) that NO voxel of the
+  // group lists gets no window at all: no box, no A tile, no MMA ("skip these negligible contributions").
+  unsigned listed = 0xffffu;
+  if (P.wtx_tab) {
+    listed = 0u;
+    for (int q = 0; q < P.Q; ++q) listed |= (tx_weight(P, q, vx.n) != 0.f ? 1u : 0u) << q;
+  }
 
   for (int li = 0; li < td.list_cnt; ++li) {
     const long long e = td.list_off + li;
     if (tid < kTcG * 16) { kmn[tid / 16][tid % 16] = INT_MAX; kmx[tid / 16][tid % 16] = INT_MIN; }
+    if (tid < kTcG) lst[tid] = 0u;
     __syncthreads();
     const float4 el = __ldg(&P.elem[list[e].x]);
     const float4 dir = P.has_dir ? __ldg(&P.edir[list[e].x]) : make_float4(0.f, 0.f, 1.f, 0.f);
@@ -630,14 +643,22 @@ tc_window_kernel(const TcDev tp, const Params P, uint2* __restrict__ list, unsig
         if (lane == 0 && lo != INT_MAX) { atomicMin(&kmn[g][q], lo); atomicMax(&kmx[g][q], hi); }
       }
     }
+    {
+      // the windows above span ALL voxels inside the aperture (a voxel that does not list q still indexes the
+      // placement table with its own sample position); only "does anybody list q" decides whether the item exists
+      const unsigned any_l = __reduce_or_sync(0xffffffffu, act ? listed : 0u);
+      if (lane == 0 && any_l) atomicOr(&lst[g], any_l);
+    }
     __syncthreads();
     if (tid < 16) {
       const int q = tid;
       unsigned flags = 0;
       int u0 = INT_MAX, uend = INT_MIN;                          // samples the item needs: [u0, uend)
       if (q < P.Q)
-        for (int gg = 0; gg < kTcG; ++gg)
+        for (int gg = 0; gg < kTcG; ++gg) {
+          if (!((lst[gg] >> q) & 1u)) kmn[gg][q] = INT_MAX;      // nobody in the group lists q (only this thread touches column q now)
           if (kmn[gg][q] != INT_MAX) { u0 = min(u0, kmn[gg][q]); uend = max(uend, kmx[gg][q] + 2); }
+        }
       bool big = false;
       if (u0 != INT_MAX) {
         big = uend - u0 > kTcBoxSmall;

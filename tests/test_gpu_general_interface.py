@@ -215,3 +215,38 @@ def test_unlisted_transmit_is_never_summed(das_lib, algo):
     plan = das.Plan.from_workload(w, storage=das.STORE_FP32, algo=algo, w_tx=wt, obs=(off, oq))
     assert plan.count_work()[1] == int(ref["count"].sum())
     plan.destroy()
+
+
+def quadrant_lists(w):
+    """A spatially selective sequence: every voxel lists the transmits whose virtual source lies in its own lateral
+    quadrant (sign of x and of y): 4 of the headline's 16 sources.  Returns (obs_off, obs_q)."""
+    gx, gy, _ = np.meshgrid(w.xs, w.ys, w.zs, indexing="ij")
+    sx, sy = np.signbit(gx.ravel()), np.signbit(gy.ravel())
+    vx, vy = np.signbit(w.tx_v[:, 0]), np.signbit(w.tx_v[:, 1])
+    mask = (vx[:, None] == sx[None, :]) & (vy[:, None] == sy[None, :])                 # [Q, N]
+    off = np.concatenate([[0], np.cumsum(mask.sum(0))]).astype(np.int64)
+    oq = np.concatenate([np.nonzero(mask[:, i])[0] for i in range(mask.shape[1])]).astype(np.int32)
+    return off, oq, mask
+
+
+@pytest.mark.timeout(300)
+def test_tc_kernel_skips_items_nobody_lists(das_lib):
+    """the sparse list "would let the kernel skip these negligible contributions".  With quadrant lists
+    most (transmit, receiver, depth group) items of a tile are listed by none of its voxels; the plan gives them no
+    window, so the batch kernel stages no box and issues no MMA for them (16 transmits, so this also runs the
+    run-time slot tracking instead of the compile-time phases).  Frames 0 and 5 against the oracle, on a block that
+    straddles all four quadrants."""
+    import oracle
+    from test_gpu_tc import make_batch
+    das = das_lib
+    w = _subgrid(3, slice(40, 88), slice(48, 80), slice(60, 72))            # 48 x 32 x 12 around the axis
+    off, oq, mask = quadrant_lists(w)
+    assert mask.sum(0).min() == 4 and mask.sum(0).max() == 4 and mask.any(1).all()
+    yb = make_batch(w.y, 8, 140)
+    got = run(das, w, das.STORE_FP16, das.ALGO_TC, das.ALGO_TC, n_frames=8, y=yb, obs=(off, oq))
+    for b in (0, 5):
+        ref = oracle.das(w, y=yb[b], obs=(off, oq))
+        emax, el2 = errors(got[b], ref)
+        assert emax <= TOL_FP16_MAX and el2 <= TOL_FP16_L2, (b, emax, el2)
+    dense = oracle.das(w, y=yb[0])
+    assert np.abs(dense - oracle.das(w, y=yb[0], obs=(off, oq))).max() > 0.05 * np.abs(dense).max()   # the lists matter
