@@ -621,7 +621,7 @@ def run_cuda(args):
 
     value = world * B * steps / (total_ms * 1e-3)
     # ncu counters of the two kernels: read from the committed summaries, never typed in here
-    prof_tc = load_profile("r2_tc_b64_full")
+    prof_tc = load_profile("r3_tc_b64_full") or load_profile("r2_tc_b64_full")
     prof_tiled = load_profile("r2_tiled_iq16_full") if (args.config == 3 and args.storage == "fp16") else None
     if B == 1:
         flops = flops1
